@@ -1,0 +1,194 @@
+/*
+ * gridff.h — C-ABI of the B200-native GridFF hot path (arxiv 2508.15522).
+ *
+ * The library implements, as hand-written CUDA for sm_100a, the data-parallel path of the paper:
+ *   substrate atoms + periodic cell + voxel size  ->  B-spline coefficient grids
+ *   positions + per-atom channel factors          ->  E_i, F_i by tricubic B-splines    (Eq.1, L128-138 Eqs.5-6)
+ *   N replicas + topology + integrator            ->  final states and energies
+ *
+ * Conventions
+ *   - Units: Å, eV, e, amu, fs.  k_e = 14.3996454784 eV·Å/e²;  1 eV/(Å·amu) = 9.648533212e-3 Å/fs².
+ *   - Every function returns 0 (GRIDFF_OK) or a negative error code; gridff_last_error() gives a thread-local
+ *     message.  No exception crosses the ABI.
+ *   - Pointers named d_* are DEVICE pointers, h_* / unprefixed array pointers are HOST pointers.
+ *   - The library never allocates, frees or keeps caller memory beyond what is stated: device buffers
+ *     (store, scratch, topology buffer, work buffers) are owned by the caller (e.g. torch tensors) and must stay
+ *     alive while the handle that refers to them is in use.  Opaque handles are small host objects owned by the
+ *     library and released by gridff_free_grid / gridff_free_molecule.
+ *   - All device work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream) and is
+ *     asynchronous unless stated.  Host input arrays are consumed before the call returns.
+ *   - Arrays are row-major, atom-major xyz.  Out-of-domain atoms are not an error (rules at gridff_eval);
+ *     a replica that produces NaN sets bit 30 of its status flag, the call still returns 0.
+ *   - There is no CPU fallback anywhere: without a CUDA device every compute entry point returns GRIDFF_ECUDA.
+ */
+#ifndef GRIDFF_H
+#define GRIDFF_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GRIDFF_OK 0
+#define GRIDFF_EINVAL (-1)        /* bad argument */
+#define GRIDFF_EUNSUPPORTED (-2)  /* e.g. non-neutral substrate with a Coulomb channel, > 64 atoms per molecule */
+#define GRIDFF_ESIZE (-3)         /* a caller buffer is too small */
+#define GRIDFF_ECUDA (-4)         /* CUDA runtime error (message in gridff_last_error) */
+
+const char* gridff_last_error(void);
+int gridff_version(void);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Grid build  (steps a1-a4; Eqs. 2-4)
+ * --------------------------------------------------------------------------------------------------------- */
+
+typedef struct gridff_grid gridff_grid;
+
+typedef enum { GRIDFF_CH_PAULI = 0, GRIDFF_CH_LONDON = 1, GRIDFF_CH_COULOMB = 2, GRIDFF_CH_ZERO = 3 } gridff_channel;
+
+typedef enum {
+    GRIDFF_LAYOUT_ZFAST = 0,  /* [x][y][z] nodes, z contiguous (the paper's order), x/y halo of 3 nodes */
+    GRIDFF_LAYOUT_BRICK = 1   /* 4x4x4-node bricks of 1 KB, bricks in [x][y][z] order, x/y halo                     */
+} gridff_layout;
+
+typedef struct {
+    double Lx, Ly;        /* periodic orthorhombic surface cell, Å                               */
+    double z_ref;         /* z of the top substrate layer                                                               */
+    double z_lo, z_hi;    /* grid z range above z_ref; node k sits at z_ref + z_lo + k*spacing                          */
+    double spacing;       /* target voxel size: nx = round(Lx/spacing), hx = Lx/nx (same for y); nz = round((z_hi-z_lo)/spacing), hz = spacing */
+    double alpha;         /* Morse alpha, 1/Å                                                         */
+    double r_cut;         /* lateral images with |a| <= ceil(r_cut/Lx), |b| <= ceil(r_cut/Ly) are summed  */
+    int n_channels;       /* 1..4; every node is stored as 4 floats (16 B), missing channels are zero                    */
+    int channel[4];       /* gridff_channel per stored component                                                        */
+    int layout;           /* gridff_layout                                                                              */
+    int l2_persist;       /* 1: ask for an L2 access-policy window over the store on the streams that use the grid      */
+} gridff_grid_desc;
+
+/* nodes per axis, spacings and origin {0, 0, z_ref+z_lo} implied by a descriptor. */
+int gridff_grid_dims(const gridff_grid_desc* desc, int dims[3], double h[3], double origin[3]);
+
+/* Bytes the caller must provide for the coefficient store (kept for the life of the grid) and for the build
+ * scratch (may be released once the stream has finished the build). */
+int gridff_grid_bytes(const gridff_grid_desc* desc, int n_sub, size_t* store_bytes, size_t* scratch_bytes);
+
+/* Sample the channels on the grid, prefilter them to interpolating cubic B-spline coefficients (cyclic in x,y;
+ * not-a-knot in z) and write the interleaved fp32 store.
+ *   sub_pos [n_sub][3], sub_e (sqrt(eps_j), eV^1/2), sub_R (Å), sub_q (e): HOST doubles; sub_q may be NULL without a
+ *   Coulomb channel.  A Coulomb channel needs |sum q| < 1e-9 e (GRIDFF_EUNSUPPORTED otherwise) and a grid that starts
+ *   above every substrate atom.  Sampling and prefilter run in fp64 on the device; the store is fp32.
+ *   Synchronises the stream once (host -> device copy of the substrate from pageable memory).                    */
+int gridff_build_grid(const gridff_grid_desc* desc, int n_sub,
+                      const double* sub_pos, const double* sub_e, const double* sub_R, const double* sub_q,
+                      void* d_store, size_t store_bytes, void* d_scratch, size_t scratch_bytes,
+                      void* cuda_stream, gridff_grid** out);
+
+/* Same, but the node samples are supplied by the caller (density-derived or imported potentials):
+ * d_samples [nx][ny][nz][n_channels] fp32 on the device. */
+int gridff_grid_from_samples(const gridff_grid_desc* desc, const float* d_samples,
+                             void* d_store, size_t store_bytes, void* d_scratch, size_t scratch_bytes,
+                             void* cuda_stream, gridff_grid** out);
+
+/* Parity hook: write the stored coefficients in canonical order, d_coef [nx][ny][nz][n_channels] fp32. */
+int gridff_grid_export(const gridff_grid* grid, float* d_coef, void* cuda_stream);
+
+int gridff_grid_info(const gridff_grid* grid, int dims[3], double h[3], double origin[3], int* n_channels, int* layout);
+
+/* Frees the handle only; d_store stays the caller's. */
+int gridff_free_grid(gridff_grid* grid);
+
+/* Per-atom channel factors of PAPER.md:L83-85 Eq. 4 with e_i = sqrt(eps_i):
+ *   coef[i] = { e_i exp(2 alpha R_i), -2 e_i exp(alpha R_i), q_i, 0 }.   HOST arrays, computed on the host in fp64. */
+int gridff_atom_coefs(double alpha, int n, const float* e, const float* R, const float* q, float* coef);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Interpolation  (step a5)
+ * --------------------------------------------------------------------------------------------------------- */
+
+/* E_i = sum_c coef[i][c] V_c(r_i),  F_i = -sum_c coef[i][c] grad V_c(r_i) for n points.
+ *   d_pos [n][3] Å, d_coef [n][4], d_E [n] eV (may be NULL), d_F [n][3] eV/Å (may be NULL): device, fp32.
+ *   x,y are wrapped into the cell.  z above the stored domain (node index >= nz-2): E = F = 0;
+ *   z below node 1: the lowest cell's polynomial is continued.                                                 */
+int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
+                float* d_E, float* d_F, void* cuda_stream);
+
+/* Same through HOST buffers: copies pos/coef to d_work, evaluates, copies E/F back, synchronises the stream.
+ * d_work needs gridff_eval_work_bytes(n) bytes. */
+size_t gridff_eval_work_bytes(long long n);
+int gridff_eval_host(const gridff_grid* grid, long long n, const float* h_pos, const float* h_coef,
+                     float* h_E, float* h_F, void* d_work, size_t work_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Fused replica step  (steps a5-a9)
+ * --------------------------------------------------------------------------------------------------------- */
+
+typedef struct {
+    int n_atoms;                                   /* 1..64 */
+    const float* mass;                             /* [n] amu */
+    const float* coef;                             /* [n][4] channel factors (gridff_atom_coefs) */
+    const float* q; const float* lj_e; const float* lj_R;   /* [n] e, sqrt(eps) eV^1/2, Å (R_ij = R_i + R_j) */
+    int n_bonds;  const int* bond;  const float* bond_k_r0;      /* [.][2] i,j;       [.][2] k (eV/Å²), r0 (Å)      E = k/2 (r-r0)²        */
+    int n_angles; const int* angle; const float* angle_k_t0;     /* [.][3] i,j,k (j centre); k (eV/rad²), theta0    E = k/2 (th-th0)²      */
+    int n_tors;   const int* tors;  const float* tors_k_n_p0;    /* [.][4] i,j,k,l;   k (eV), n, phi0               E = k [1+cos(n phi-phi0)] */
+    const unsigned char* excl;                     /* [n][n], 1 = pair excluded from LJ + Coulomb; NULL = all excluded */
+    /* restart generator (used with integrator.restart = 1) */
+    int n_rot; const int* rot_bond;                /* [.][2] rotatable bonds j0 -> j1 */
+    const unsigned char* rot_mask;                 /* [.][n] 1 = atom turns with j1 */
+    const float* ref_pos;                          /* [n][3] template conformation */
+} gridff_topology;                                 /* HOST arrays; copied by gridff_create_molecule */
+
+typedef struct gridff_molecule gridff_molecule;
+
+size_t gridff_molecule_bytes(const gridff_topology* topo);
+/* Pack the topology into the caller's device buffer d_buf (>= gridff_molecule_bytes).  Synchronises the stream. */
+int gridff_create_molecule(const gridff_topology* topo, void* d_buf, size_t buf_bytes, void* cuda_stream,
+                           gridff_molecule** out);
+int gridff_free_molecule(gridff_molecule* mol);
+
+typedef struct {
+    int kind;                 /* 0 velocity Verlet, 1 FIRE (ref 72) */
+    int n_steps;              /* steps per launch (FIRE: upper bound) */
+    float dt;                 /* fs (FIRE: initial dt) */
+    float f_tol;              /* FIRE stops when max_i |F_i| < f_tol, eV/Å */
+    float dt_max, f_inc, f_dec, a_start, f_a; int n_min;    /* FIRE parameters; defaults 10 dt, 1.1, 0.5, 0.1, 0.99, 5 */
+    float max_step;           /* FIRE: cap on the largest atomic displacement per step, Å; 0 = none */
+    int restart;              /* FIRE: 0 stop when converged; 1 record the minimum and re-seed from Philox4x32-10(seed, replica, restart#) */
+    unsigned long long seed;
+    float z_ref, place_z_lo, place_z_hi, place_z_min, clash;   /* restart placement (3, 6, 2 Å above z_ref; clash factor 0.4) */
+    int variant;              /* kernel variant: 0 = default (library's choice), 1 = re-gather every step, 2 = cell-cached stencils */
+} gridff_integrator;
+
+/* Advance n_rep independent replicas of one molecule for integ->n_steps steps in ONE launch sequence without host
+ * round-trips: per step, grid forces by interpolation + intramolecular terms + integrator.
+ *   d_pos, d_vel   [n_rep][n][3]  in/out, fp32
+ *   d_fire         [n_rep][4]     in/out FIRE scalars {dt, a, steps since P<=0, restarts done}; dt <= 0 = fresh.  May be NULL (VV, or fresh FIRE)
+ *   d_energy       [n_rep][8]     out: grid ch0, ch1, ch2, bond, angle, torsion, non-bonded, kinetic (eV) at the final state.  May be NULL
+ *   d_status       [n_rep][2]     out: {steps taken, converged flag (restart=0) or minima recorded (restart=1)}.  May be NULL
+ *   d_minima       [cap][4+3n]    out, restart=1: {replica, restart#, steps, E_total, positions}; d_n_minima (1 int, device, caller zeroes it)
+ *                                 counts records (may exceed cap; excess dropped).  May be NULL
+ * `grid` may be NULL (gas-phase molecule).                                                                          */
+int gridff_run_replicas(const gridff_grid* grid, const gridff_molecule* mol, const gridff_integrator* integ, int n_rep,
+                        float* d_pos, float* d_vel, float* d_fire, float* d_energy, int* d_status,
+                        float* d_minima, int minima_cap, int* d_n_minima, void* cuda_stream);
+
+/* Same through HOST buffers (pinned or pageable): copies pos/vel(/fire) to d_work, runs, copies pos/vel/fire/energy/
+ * status back, synchronises the stream.  d_work needs gridff_run_work_bytes(mol, n_rep) bytes. */
+size_t gridff_run_work_bytes(const gridff_molecule* mol, int n_rep);
+int gridff_run_replicas_host(const gridff_grid* grid, const gridff_molecule* mol, const gridff_integrator* integ, int n_rep,
+                             float* h_pos, float* h_vel, float* h_fire, float* h_energy, int* h_status,
+                             void* d_work, size_t work_bytes, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------------------
+ * Measurement helpers (roofline denominators; not part of the method)
+ * --------------------------------------------------------------------------------------------------------- */
+
+/* Read `bytes` of d_buf `iters` times with coalesced 16-byte loads (mode 0) or with the 64-byte-row gather pattern of
+ * the stencil at random offsets (mode 1); one launch.  d_sink: >= 4 bytes.  Used to measure L2 / HBM read bandwidth. */
+int gridff_probe_read(const void* d_buf, size_t bytes, int iters, int mode, void* d_sink, void* cuda_stream);
+
+/* Number of kernel launches the library has enqueued since it was loaded (for bench.py's gpu_launches). */
+long long gridff_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
