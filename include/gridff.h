@@ -111,6 +111,11 @@ int gridff_atom_coefs(double alpha, int n, const float* e, const float* R, const
 int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
                 float* d_E, float* d_F, void* cuda_stream);
 
+/* Same with an explicit kernel variant (layout / gather study): 0 = library default, 1 = one thread per point
+ * (64 independent 16-byte loads), 2 = warp-cooperative row gather.  A brick-layout grid always uses its own kernel. */
+int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
+                        float* d_E, float* d_F, int variant, void* cuda_stream);
+
 /* Same through HOST buffers: copies pos/coef to d_work, evaluates, copies E/F back, synchronises the stream.
  * d_work needs gridff_eval_work_bytes(n) bytes. */
 size_t gridff_eval_work_bytes(long long n);
@@ -154,7 +159,7 @@ typedef struct {
     int restart;              /* FIRE: 0 stop when converged; 1 record the minimum and re-seed from Philox4x32-10(seed, replica, restart#) */
     unsigned long long seed;
     float z_ref, place_z_lo, place_z_hi, place_z_min, clash;   /* restart placement (3, 6, 2 Å above z_ref; clash factor 0.4) */
-    int variant;              /* kernel variant: 0 = default (library's choice), 1 = re-gather every step, 2 = cell-cached stencils */
+    int variant;              /* kernel variant: 0 = default (library's choice), 1 = one thread per atom gathers its 64 nodes, 2 = warp-cooperative row gather */
 } gridff_integrator;
 
 /* Advance n_rep independent replicas of one molecule for integ->n_steps steps in ONE launch sequence without host

@@ -1,0 +1,203 @@
+// gridff_eval.cu — gridff_eval (step a5) and the bandwidth probe.  PAPER.md:L128-138; DESIGN.md §5.
+#include "gridff_interp.cuh"
+#include <stdio.h>
+
+using namespace gridff;
+
+namespace {
+
+// variant 1: one thread per point, 64 independent 16-byte loads (the paper's per-atom loop moved to a thread)
+__global__ void __launch_bounds__(128) k_eval_direct(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
+                                                     float* __restrict__ E, float* __restrict__ F) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const Stencil s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2]);
+    float e, fx, fy, fz;
+    interp_direct(g, s, coef[p], e, fx, fy, fz);
+    if (E) E[p] = e;
+    if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
+}
+
+// variant 2: warp-cooperative row gather.  A warp owns 32 consecutive points; for each of them 4 lanes fetch each 64-byte
+// stencil row (8 rows per LDG.128), fold the channels and park the 64 scalars in shared memory; then every lane contracts
+// its own point from the (swizzled) tile.
+constexpr int kEvalWarps = 4;
+
+__global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
+                                                               float* __restrict__ E, float* __restrict__ F) {
+    __shared__ __align__(16) float s_tile[kEvalWarps][32 * 64];
+    __shared__ __align__(16) float4 s_cf[kEvalWarps][32];
+    __shared__ unsigned s_base[kEvalWarps][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const long long p = ((long long)blockIdx.x * kEvalWarps + w) * 32 + lane;
+    Stencil s; s.base = kNoStencil; s.tx = s.ty = s.tz = 0.f;
+    float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2]); cf = coef[p]; }
+    s_base[w][lane] = s.base; s_cf[w][lane] = cf;
+    __syncwarp();
+    float* tile = s_tile[w];
+#pragma unroll 8
+    for (int q = 0; q < 32; ++q) {
+        const unsigned b = s_base[w][q];
+        if (b != kNoStencil) gather_rows(g, b, s_cf[w][q], lane, q, tile);
+    }
+    __syncwarp();
+    if (p >= n) return;
+    float e, fx, fy, fz;
+    interp_tile(g, s, lane, tile, e, fx, fy, fz);
+    if (E) E[p] = e;
+    if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
+}
+
+// brick layout, thread per point (layout study)
+__device__ __forceinline__ size_t brick_index(const GridGeom& g, int s_x, int s_y, int iz) {
+    const int by_n = (g.sy + 3) >> 2, bz_n = g.nzp >> 2;
+    const size_t brick = ((size_t)(s_x >> 2) * by_n + (s_y >> 2)) * bz_n + (iz >> 2);
+    return brick * 64 + (size_t)(((s_x & 3) << 4) | ((s_y & 3) << 2) | (iz & 3));
+}
+
+__global__ void __launch_bounds__(128) k_eval_brick(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
+                                                    float* __restrict__ E, float* __restrict__ F) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    int ix, iy, iz; float tx, ty, tz;
+    cell_periodic(pos[3 * p], g.inv_hx_hi, g.inv_hx_lo, g.nx, ix, tx);
+    cell_periodic(pos[3 * p + 1], g.inv_hy_hi, g.inv_hy_lo, g.ny, iy, ty);
+    float e = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
+    if (cell_z(pos[3 * p + 2], g, iz, tz)) {
+        const float4 cf = coef[p];
+        Contract C; C.init(tx, ty, tz);
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                float c[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) c[k] = fold4(cf, __ldg(g.store + brick_index(g, ix + a, iy + b, iz - 1 + k)));
+                C.row(a, b, c[0], c[1], c[2], c[3]);
+            }
+        e = C.e; fx = -C.gx * g.inv_hx; fy = -C.gy * g.inv_hy; fz = -C.gz * g.inv_hz;
+    }
+    if (E) E[p] = e;
+    if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
+}
+
+// ---- bandwidth probe ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned hash32(unsigned x) {
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+__global__ void __launch_bounds__(256) k_probe_stream(const float4* __restrict__ buf, size_t n16, int iters, float* sink) {
+    float acc = 0.f;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (int it = 0; it < iters; ++it) {
+        size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+        for (; i + 3 * stride < n16; i += 4 * stride) {
+            const float4 a = buf[i], b = buf[i + stride], c = buf[i + 2 * stride], d = buf[i + 3 * stride];
+            acc += (a.x + b.y) + (c.z + d.w);
+        }
+        for (; i < n16; i += stride) acc += buf[i].x;
+    }
+    if (acc == 1.2345678e-30f) *sink = acc;
+}
+
+// 4 lanes read one 64-byte row at a random 16-byte-aligned offset (the stencil's access granule)
+__global__ void __launch_bounds__(256) k_probe_rows(const float4* __restrict__ buf, size_t n16, int iters, float* sink) {
+    float acc = 0.f;
+    const unsigned quad = (blockIdx.x * blockDim.x + threadIdx.x) >> 2, k = threadIdx.x & 3;
+    const unsigned nquads = (gridDim.x * blockDim.x) >> 2;
+    const size_t rows = n16 / 4;                   // rows of 64 B to read per pass
+    const unsigned span = (unsigned)(n16 - 4);
+    for (int it = 0; it < iters; ++it) {
+        for (size_t r = quad; r < rows; r += (size_t)nquads * 4) {
+            unsigned h = hash32((unsigned)r * 2654435761u + (unsigned)it);
+            float4 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const size_t rr = r + (size_t)u * nquads;
+                if (rr < rows) { v[u] = buf[(size_t)(h % span) + k]; } else v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                h = hash32(h + 0x9e3779b9u);
+            }
+            acc += (v[0].x + v[1].y) + (v[2].z + v[3].w);
+        }
+    }
+    if (acc == 1.2345678e-30f) *sink = acc;
+}
+
+}  // namespace
+
+
+extern "C" {
+
+int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F,
+                        int variant, void* cuda_stream) {
+    if (!grid) { set_error("grid is NULL"); return GRIDFF_EINVAL; }
+    if (n < 0) { set_error("n < 0"); return GRIDFF_EINVAL; }
+    if (n == 0) return GRIDFF_OK;
+    if (!d_pos || !d_coef) { set_error("d_pos / d_coef is NULL"); return GRIDFF_EINVAL; }
+    if ((uintptr_t)d_coef & 15) { set_error("d_coef must be 16-byte aligned"); return GRIDFF_EINVAL; }
+    const GridGeom& G = grid->geom;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+    if (G.layout == GRIDFF_LAYOUT_BRICK) {
+        e = launch_with_window(grid, k_eval_brick, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    } else if (variant == 1) {
+        e = launch_with_window(grid, k_eval_direct, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    } else if (variant == 0 || variant == 2) {
+        const long long per_block = kEvalWarps * 32;
+        e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    } else { set_error("unknown eval variant %d", variant); return GRIDFF_EINVAL; }
+    count_launch();
+    if (e != cudaSuccess) return cuda_fail(e, "gridff_eval launch");
+    return GRIDFF_OK;
+}
+
+int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, void* cuda_stream) {
+    return gridff_eval_variant(grid, n, d_pos, d_coef, d_E, d_F, 0, cuda_stream);
+}
+
+size_t gridff_eval_work_bytes(long long n) {
+    if (n < 0) n = 0;
+    return (size_t)n * (12 + 16 + 4 + 12) + 256;
+}
+
+int gridff_eval_host(const gridff_grid* grid, long long n, const float* h_pos, const float* h_coef, float* h_E, float* h_F,
+                     void* d_work, size_t work_bytes, void* cuda_stream) {
+    if (!grid) { set_error("grid is NULL"); return GRIDFF_EINVAL; }
+    if (n < 0 || !h_pos || !h_coef) { set_error("bad n / host pointers"); return GRIDFF_EINVAL; }
+    if (n == 0) return GRIDFF_OK;
+    if (!d_work || work_bytes < gridff_eval_work_bytes(n)) { set_error("d_work too small"); return GRIDFF_ESIZE; }
+    if ((uintptr_t)d_work & 255) { set_error("d_work must be 256-byte aligned"); return GRIDFF_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    char* w = (char*)d_work;
+    float* d_coef = (float*)w;                       // [n][4]  (16-byte aligned)
+    float* d_pos = (float*)(w + (size_t)n * 16);     // [n][3]
+    float* d_F = (float*)(w + (size_t)n * 28);       // [n][3]
+    float* d_E = (float*)(w + (size_t)n * 40);       // [n]
+    GRIDFF_CUDA(cudaMemcpyAsync(d_coef, h_coef, (size_t)n * 16, cudaMemcpyHostToDevice, st));
+    GRIDFF_CUDA(cudaMemcpyAsync(d_pos, h_pos, (size_t)n * 12, cudaMemcpyHostToDevice, st));
+    int rc = gridff_eval(grid, n, d_pos, d_coef, h_E ? d_E : nullptr, h_F ? d_F : nullptr, cuda_stream);
+    if (rc) return rc;
+    if (h_E) GRIDFF_CUDA(cudaMemcpyAsync(h_E, d_E, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
+    if (h_F) GRIDFF_CUDA(cudaMemcpyAsync(h_F, d_F, (size_t)n * 12, cudaMemcpyDeviceToHost, st));
+    GRIDFF_CUDA(cudaStreamSynchronize(st));
+    return GRIDFF_OK;
+}
+
+int gridff_probe_read(const void* d_buf, size_t bytes, int iters, int mode, void* d_sink, void* cuda_stream) {
+    if (!d_buf || !d_sink || bytes < 4096 || iters < 1) { set_error("bad probe arguments"); return GRIDFF_EINVAL; }
+    if ((uintptr_t)d_buf & 15) { set_error("d_buf must be 16-byte aligned"); return GRIDFF_EINVAL; }
+    if (bytes / 16 > 0xFFFFFFF0ull && mode == 1) { set_error("row probe supports < 64 GB"); return GRIDFF_EINVAL; }
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (mode == 0) k_probe_stream<<<sms * 8, 256, 0, st>>>((const float4*)d_buf, bytes / 16, iters, (float*)d_sink);
+    else if (mode == 1) k_probe_rows<<<sms * 8, 256, 0, st>>>((const float4*)d_buf, bytes / 16, iters, (float*)d_sink);
+    else { set_error("unknown probe mode %d", mode); return GRIDFF_EINVAL; }
+    GRIDFF_LAUNCH_CHECK("gridff_probe_read");
+    return GRIDFF_OK;
+}
+
+}  // extern "C"

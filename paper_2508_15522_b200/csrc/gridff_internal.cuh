@@ -1,0 +1,104 @@
+// gridff_internal.cuh — shared declarations of the CUDA GridFF library (sm_100a).  Product code: shares nothing
+// with oracle/.  Public surface is include/gridff.h; everything here is internal.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/gridff.h"
+
+namespace gridff {
+
+constexpr double kKe = 14.3996454784;      // eV·Å/e²
+constexpr double kAcc = 9.648533212e-3;    // 1 eV/(Å·amu) in Å/fs²
+constexpr int kMaxAtoms = 64;
+constexpr int kHalo = 3;                   // stored x/y extent = n + 3: stored index s holds node (s - 1) mod n
+
+// Geometry of the fp32 coefficient store, passed by value to every kernel that interpolates.
+// Node (jx, jy, jz), jx in [-1, nx+1], is the float4 at  store[((jx+1) * sy + (jy+1)) * nzp + jz]   (ZFAST)
+struct GridGeom {
+    int nx, ny, nz;              // nodes per axis
+    int sx, sy, nzp;             // stored extents: nx+3, ny+3, nz rounded up to 8 nodes (128 B lines)
+    int layout;
+    int n_channels;
+    // 1/h split into hi + lo floats so that t = fma(x, hi, -i) + x*lo keeps ~1e-7 of a cell at any |x|
+    float inv_hx_hi, inv_hx_lo, inv_hy_hi, inv_hy_lo, inv_hz_hi, inv_hz_lo;
+    float z0_hi, z0_lo;          // z of node 0 (z_ref + z_lo), split
+    float inv_hx, inv_hy, inv_hz;
+    const float4* store;
+};
+
+struct MolDev;   // packed molecule in device memory (gridff_replica.cu)
+
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);
+void count_launch(int n = 1);
+
+#define GRIDFF_CUDA(call)                                        \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return gridff::cuda_fail(e__, #call); \
+    } while (0)
+
+#define GRIDFF_LAUNCH_CHECK(name)                                \
+    do {                                                         \
+        gridff::count_launch();                                  \
+        cudaError_t e__ = cudaGetLastError();                    \
+        if (e__ != cudaSuccess) return gridff::cuda_fail(e__, name); \
+    } while (0)
+
+// ---- B-spline weights (Eqs. 5-6; polynomial pieces of B(t+1-j), j = 0..3) -------------------
+__device__ __forceinline__ void bspline_w(float t, float w[4], float d[4]) {
+    const float s = 1.0f - t, t2 = t * t, s2 = s * s;
+    const float k6 = 1.0f / 6.0f;
+    w[0] = s2 * s * k6;
+    w[3] = t2 * t * k6;
+    w[1] = fmaf(t2, fmaf(0.5f, t, -1.0f), 2.0f / 3.0f);      // t^3/2 - t^2 + 2/3
+    w[2] = fmaf(s2, fmaf(0.5f, s, -1.0f), 2.0f / 3.0f);      // mirror image: (1-t)
+    d[0] = -0.5f * s2;
+    d[3] = 0.5f * t2;
+    d[1] = t * fmaf(1.5f, t, -2.0f);                          // 3/2 t^2 - 2 t
+    d[2] = -s * fmaf(1.5f, s, -2.0f);
+}
+
+// cell index (wrapped into [0,n)) and fraction along a periodic axis
+__device__ __forceinline__ void cell_periodic(float x, float inv_hi, float inv_lo, int n, int& i, float& t) {
+    float fi = floorf(x * inv_hi);
+    float tt = fmaf(x, inv_hi, -fi) + x * inv_lo;
+    if (tt < 0.0f) { tt += 1.0f; fi -= 1.0f; }
+    if (tt >= 1.0f) { tt -= 1.0f; fi += 1.0f; }
+    int ii = (int)fi % n;                 // |fi| < 2^24 for any sane coordinate; NaN -> 0
+    if (ii < 0) ii += n;
+    i = ii; t = tt;
+}
+
+// z axis: returns false when the point is above the stored domain (E = F = 0, gridff.h); below node 1 the lowest
+// cell's polynomial is continued (t < 0).
+__device__ __forceinline__ bool cell_z(float z, const GridGeom& g, int& i, float& t) {
+    const float dz = (z - g.z0_hi) - g.z0_lo;
+    const float q = dz * g.inv_hz_hi;
+    if (!(q < (float)(g.nz - 2))) {
+        // q rounds to nz-2 from below only within 1 ulp: treat as above as well (E there is ~0 by construction)
+        return false;
+    }
+    float fi = floorf(q);
+    fi = fminf(fmaxf(fi, 1.0f), (float)(g.nz - 3));
+    t = fmaf(dz, g.inv_hz_hi, -fi) + dz * g.inv_hz_lo;
+    i = (int)fi;
+    return true;
+}
+
+// stored-array offset (in float4 nodes) of the stencil corner (ix-1, iy-1, iz-1) in the ZFAST layout
+__device__ __forceinline__ size_t corner_zfast(const GridGeom& g, int ix, int iy, int iz) {
+    return ((size_t)ix * g.sy + iy) * g.nzp + (iz - 1);
+}
+
+}  // namespace gridff
+
+// opaque handles ------------------------------------------------------------------------------------------------
+struct gridff_grid {
+    gridff::GridGeom geom;
+    gridff_grid_desc desc;
+    double h[3], origin[3];
+    size_t store_bytes;
+    int l2_window_ok;     // 1 when an access-policy window could be applied
+};

@@ -1,0 +1,149 @@
+// gridff_interp.cuh — device-side tricubic B-spline interpolation (step a5; Eqs. 5-6, L53 Eq. 1).
+//   E_i = sum_c coef_ic V_c(r_i),  F_i = -sum_c coef_ic grad V_c(r_i),  V_c = sum_{abk} w_a(tx) w_b(ty) w_k(tz) b_c[node abk]
+// The channel factors are folded into the nodes first (one scalar per node, 64 per atom), then the tensor product is
+// contracted z -> y -> x (the paper's 16+4+1 order), carrying the three derivative sums along.
+#pragma once
+#include "gridff_internal.cuh"
+
+namespace gridff {
+
+struct Stencil {           // where an atom sits in the grid
+    unsigned base;         // float4 offset of node (ix-1, iy-1, iz-1) in the ZFAST store; 0xFFFFFFFF = above the domain
+    float tx, ty, tz;
+};
+constexpr unsigned kNoStencil = 0xFFFFFFFFu;
+
+__device__ __forceinline__ Stencil locate(const GridGeom& g, float x, float y, float z) {
+    Stencil s; int ix, iy, iz;
+    cell_periodic(x, g.inv_hx_hi, g.inv_hx_lo, g.nx, ix, s.tx);
+    cell_periodic(y, g.inv_hy_hi, g.inv_hy_lo, g.ny, iy, s.ty);
+    if (cell_z(z, g, iz, s.tz)) s.base = (unsigned)corner_zfast(g, ix, iy, iz);
+    else { s.base = kNoStencil; s.tz = 0.f; }
+    return s;
+}
+
+__device__ __forceinline__ float fold4(const float4 c, const float4 n) {
+    return fmaf(c.x, n.x, fmaf(c.y, n.y, fmaf(c.z, n.z, c.w * n.w)));
+}
+
+// Accumulator for the separable contraction.  Feed the 16 rows in order r = 4a + b, each as 4 folded node values
+// along z; finish() returns E and dE/d(cell units).
+struct Contract {
+    float wx[4], dx[4], wy[4], dy[4], wz[4], dz[4];
+    float pa, pya, pza, e, gx, gy, gz;
+    __device__ __forceinline__ void init(float tx, float ty, float tz) {
+        bspline_w(tx, wx, dx); bspline_w(ty, wy, dy); bspline_w(tz, wz, dz);
+        e = gx = gy = gz = 0.f; pa = pya = pza = 0.f;
+    }
+    __device__ __forceinline__ void row(int a, int b, float c0, float c1, float c2, float c3) {
+        const float s = fmaf(wz[0], c0, fmaf(wz[1], c1, fmaf(wz[2], c2, wz[3] * c3)));
+        const float sz = fmaf(dz[0], c0, fmaf(dz[1], c1, fmaf(dz[2], c2, dz[3] * c3)));
+        pa = fmaf(wy[b], s, pa); pya = fmaf(dy[b], s, pya); pza = fmaf(wy[b], sz, pza);
+        if (b == 3) {
+            e = fmaf(wx[a], pa, e); gx = fmaf(dx[a], pa, gx); gy = fmaf(wx[a], pya, gy); gz = fmaf(wx[a], pza, gz);
+            pa = pya = pza = 0.f;
+        }
+    }
+};
+
+// thread-per-atom evaluation straight from the store (ZFAST): 64 independent 16-byte loads
+__device__ __forceinline__ void interp_direct(const GridGeom& g, const Stencil& s, const float4 cf, float& E, float& Fx, float& Fy, float& Fz) {
+    if (s.base == kNoStencil) { E = Fx = Fy = Fz = 0.f; return; }
+    Contract C; C.init(s.tx, s.ty, s.tz);
+    const float4* base = g.store + s.base;
+    const int rs = g.nzp, ps = g.sy * g.nzp;
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const float4* row = base + a * ps + b * rs;
+            const float4 n0 = __ldg(row), n1 = __ldg(row + 1), n2 = __ldg(row + 2), n3 = __ldg(row + 3);
+            C.row(a, b, fold4(cf, n0), fold4(cf, n1), fold4(cf, n2), fold4(cf, n3));
+        }
+    }
+    E = C.e; Fx = -C.gx * g.inv_hx; Fy = -C.gy * g.inv_hy; Fz = -C.gz * g.inv_hz;
+}
+
+// per-channel values V_c (no gradient) — used for the energy report only
+__device__ __forceinline__ float4 interp_channels(const GridGeom& g, const Stencil& s) {
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (s.base == kNoStencil) return v;
+    float wx[4], wy[4], wz[4], d[4];
+    bspline_w(s.tx, wx, d); bspline_w(s.ty, wy, d); bspline_w(s.tz, wz, d);
+    const float4* base = g.store + s.base;
+    const int rs = g.nzp, ps = g.sy * g.nzp;
+    for (int a = 0; a < 4; ++a) {
+        float4 pa = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int b = 0; b < 4; ++b) {
+            const float4* row = base + a * ps + b * rs;
+            float4 sr = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const float4 n = __ldg(row + k);
+                sr.x = fmaf(wz[k], n.x, sr.x); sr.y = fmaf(wz[k], n.y, sr.y); sr.z = fmaf(wz[k], n.z, sr.z); sr.w = fmaf(wz[k], n.w, sr.w);
+            }
+            pa.x = fmaf(wy[b], sr.x, pa.x); pa.y = fmaf(wy[b], sr.y, pa.y); pa.z = fmaf(wy[b], sr.z, pa.z); pa.w = fmaf(wy[b], sr.w, pa.w);
+        }
+        v.x = fmaf(wx[a], pa.x, v.x); v.y = fmaf(wx[a], pa.y, v.y); v.z = fmaf(wx[a], pa.z, v.z); v.w = fmaf(wx[a], pa.w, v.w);
+    }
+    return v;
+}
+
+// ---- warp-cooperative gather ------------------------------------------------------------------------------------
+// A stencil is 16 rows (a, b) of 4 z-nodes = 64 contiguous bytes each.  Four lanes read one row, so one LDG.128 of the warp
+// fetches 8 whole rows; two of them fetch the stencil.  Each lane folds its node with the atom's channel factors and stores one
+// scalar into a per-warp tile  tile[slot][64]  (slot = atom within the batch).  16-byte chunks are XOR-swizzled with the slot so
+// that the owner's LDS.128 reads (one lane per slot) are bank-conflict free.
+__device__ __forceinline__ int tile_word(int slot, int e /*0..63 = 4*row + k*/) {
+    return slot * 64 + ((((e >> 2) ^ (slot & 15)) << 2) | (e & 3));
+}
+
+__device__ __forceinline__ void gather_rows(const GridGeom& g, unsigned base, const float4 cf, int lane, int slot, float* tile) {
+    const int k = lane & 3, r0 = lane >> 2;                // rows r0 (a = r0>>2 in {0,1}) and r0 + 8 (a in {2,3})
+    const int a0 = r0 >> 2, b = r0 & 3;
+    const int rs = g.nzp, ps = g.sy * g.nzp;
+    const float4* p = g.store + base + a0 * ps + b * rs + k;
+    const float4 n0 = __ldg(p), n1 = __ldg(p + 2 * ps);
+    tile[tile_word(slot, lane)] = fold4(cf, n0);
+    tile[tile_word(slot, lane + 32)] = fold4(cf, n1);
+}
+
+// owner-side evaluation from the tile (after __syncwarp)
+__device__ __forceinline__ void interp_tile(const GridGeom& g, const Stencil& s, int slot, const float* tile, float& E, float& Fx, float& Fy, float& Fz) {
+    if (s.base == kNoStencil) { E = Fx = Fy = Fz = 0.f; return; }
+    Contract C; C.init(s.tx, s.ty, s.tz);
+    const float4* t4 = reinterpret_cast<const float4*>(tile) + slot * 16;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const float4 c = t4[r ^ (slot & 15)];
+        C.row(r >> 2, r & 3, c.x, c.y, c.z, c.w);
+    }
+    E = C.e; Fx = -C.gx * g.inv_hx; Fy = -C.gy * g.inv_hy; Fz = -C.gz * g.inv_hz;
+}
+
+// launch with an optional L2 access-policy window over the coefficient store (north_star: "pinned in the B200 L2")
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_with_window(const gridff_grid* grid, void (*kernel)(KArgs...), dim3 gdim, dim3 bdim, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = gdim; cfg.blockDim = bdim; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    int na = 0;
+    if (grid && grid->l2_window_ok) {
+        int dev = 0, max_window = 0, max_persist = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
+        cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
+        size_t win = grid->store_bytes < (size_t)max_window ? grid->store_bytes : (size_t)max_window;
+        attr[0].id = cudaLaunchAttributeAccessPolicyWindow;
+        attr[0].val.accessPolicyWindow.base_ptr = (void*)grid->geom.store;
+        attr[0].val.accessPolicyWindow.num_bytes = win;
+        attr[0].val.accessPolicyWindow.hitRatio = win <= (size_t)max_persist ? 1.0f : (float)max_persist / (float)win;
+        attr[0].val.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+        attr[0].val.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+        na = 1;
+    }
+    cfg.attrs = attr; cfg.numAttrs = na;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
+}  // namespace gridff
