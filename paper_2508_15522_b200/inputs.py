@@ -280,12 +280,13 @@ def _random_rotations(rng, n):
                      np.stack([2 * (x * z - y * w), 2 * (y * z + x * w), 1 - 2 * (x * x + y * y)], -1)], 1)
 
 
-def _twist(pos, topo, rng, clash=0.6, tries=32):
+def _twist(pos, topo, rng, clash=0.6, tries=256):
     """random dihedral about every rotatable bond; re-draw while a non-excluded pair is closer than
-    clash * (R_i + R_j)."""
+    clash * (R_i + R_j); if no draw passes, the least-clashing one is kept."""
     n = topo["n_atoms"]
     Rsum = topo["lj_R"][:, None].astype(np.float64) + topo["lj_R"][None, :]
     free = topo["excl"] == 0
+    best, best_gap = None, -1.0
     for _ in range(tries):
         p = pos.copy()
         for b, (j0, j1) in enumerate(topo["rot_bond"]):
@@ -295,9 +296,12 @@ def _twist(pos, topo, rng, clash=0.6, tries=32):
             v = p[sel] - p[j0]
             p[sel] = p[j0] + v * math.cos(ang) + np.cross(ax, v) * math.sin(ang) + np.outer(v @ ax, ax) * (1 - math.cos(ang))
         d = np.linalg.norm(p[:, None, :] - p[None, :, :], axis=-1)
-        if not np.any(free & (d < clash * Rsum)):
+        gap = float(np.min(np.where(free, d / Rsum, np.inf)))
+        if gap >= clash:
             return p
-    return p
+        if gap > best_gap:
+            best, best_gap = p, gap
+    return best
 
 
 def place_replicas(topo, n_rep, Lx, Ly, z_ref, seed, z_lo=3.0, z_hi=6.0, z_min=2.0, twist=False):

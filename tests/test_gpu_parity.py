@@ -241,24 +241,46 @@ def basin_match(Eg, xg, Eo, xo, Lx, Ly):
 
 @pytest.mark.parametrize("variant", [1, 2])
 def test_fire_relaxation_config0(api, orc, variant):
-    """config 0 (benzene, 2 Morse channels) on the small slab: 48 replicas x 1000 FIRE steps"""
+    """config 0 (benzene, 2 Morse channels) on the small slab, 48 replicas.  (a) the config as stated: 1000 FIRE steps, dt0 0.5 fs,
+    f_tol 1e-3 — with real masses few replicas converge that fast (DESIGN.md R13), so the final states are compared;
+    (b) dt0 1 fs, dt_max 20 fs, f_tol 1e-3, 12000 steps: most replicas converge; flags, step counts and basins are compared.
+    (The relaxation path itself is chaotic — a P <= 0 decision taken one step apart changes dt for the rest of the run — so only the
+    end states are compared; a loose f_tol leaves the stopping point along soft modes undefined to more than the 0.1 Å of the
+    basin criterion, hence the tight tolerance.)"""
     cfg = small_config(0, n_rep=48)
     og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
     g = gpu_grid(api, cfg["sub"], cfg["desc"])
     ot, mol = oracle_side(orc, cfg, og), gpu_side(api, cfg)
     vel = np.zeros_like(cfg["pos"])
+    e_start = r_start_energy(api, g, mol, cfg)
+    Lx, Ly = cfg["desc"]["Lx"], cfg["desc"]["Ly"]
+    # (a)
     r = run_gpu(api, g, mol, api.make_integrator("fire", 1000, 0.5, f_tol=1e-3, variant=variant), cfg["pos"], vel, fire=np.zeros((48, 4), np.float32))
     o = orc.run_replicas(og, ot, orc.make_integrator("fire", 1000, 0.5, f_tol=1e-3), cfg["pos"], vel)
     Eg, Eo = r["energy"][:, :7].astype(np.float64).sum(1), o["energy"][:, :7].sum(1)
-    assert np.all(Eg <= r_start_energy(api, g, mol, cfg) + 1e-6)          # relaxed E <= starting E
+    assert np.all(Eg <= e_start + 1e-6)                                   # relaxed E <= starting E
+    assert np.all(np.abs(r["energy"][:, 7]) < 1.0)
+    same = basin_match(Eg, r["pos"], Eo, o["pos"], Lx, Ly)
+    print("config 0 as stated: %d/48 replicas end in the oracle's state (|dE| < 1e-3 eV, RMSD < 0.1 Å); converged gpu %d oracle %d"
+          % (same.sum(), (r["status"][:, 1] == 1).sum(), (o["status"][:, 1] == 1).sum()))
+    assert same.mean() >= 0.9, same.mean()
+    # (b)
+    kw = dict(f_tol=1e-3, dt_max=20.0)
+    r = run_gpu(api, g, mol, api.make_integrator("fire", 12000, 1.0, variant=variant, **kw), cfg["pos"], vel, fire=np.zeros((48, 4), np.float32))
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 12000, 1.0, **kw), cfg["pos"], vel)
+    Eg, Eo = r["energy"][:, :7].astype(np.float64).sum(1), o["energy"][:, :7].sum(1)
     conv_g, conv_o = r["status"][:, 1] == 1, o["status"][:, 1] == 1
     both = conv_g & conv_o
-    assert both.sum() >= 0.8 * max(conv_o.sum(), 1), (conv_g.sum(), conv_o.sum())
-    same = basin_match(Eg, r["pos"], Eo, o["pos"], cfg["desc"]["Lx"], cfg["desc"]["Ly"])
-    # identical minimum-energy basin for relaxed replicas (north_star); a bifurcation fraction is reported, not hidden
-    frac = same[both].mean()
-    print("basin match %d/%d converged replicas" % (same[both].sum(), both.sum()))
-    assert frac >= 0.9, frac
+    assert conv_o.sum() >= 20 and both.sum() >= 0.8 * conv_o.sum(), (conv_g.sum(), conv_o.sum())
+    # a converged replica stops early and its state satisfies the criterion when re-evaluated in fp64
+    assert np.all(r["status"][conv_g, 0] < 12000)
+    for rep in np.nonzero(conv_g)[0][:8]:
+        _, F = orc.forces(og, ot, r["pos"][rep])
+        assert np.sqrt((F ** 2).sum(1)).max() < 1e-3 * 1.05
+    same = basin_match(Eg, r["pos"], Eo, o["pos"], Lx, Ly)
+    # identical minimum-energy basin for relaxed replicas (north_star); the bifurcation fraction is reported, not hidden
+    print("basin match %d/%d replicas converged on both sides" % (same[both].sum(), both.sum()))
+    assert same[both].mean() >= 0.9, same[both].mean()
 
 
 def r_start_energy(api, g, mol, cfg):
@@ -318,19 +340,20 @@ def test_restart_generator_matches_oracle(api, orc):
 def test_fire_restart_basins_config2(api, orc):
     """config 2 on the small slab: relax -> record -> re-seed.  Minima are matched by (replica, restart#); restart conformations
     are the same on both sides, so each pair starts from the same state."""
-    cfg = small_config(2, n_rep=24)
+    cfg = small_config(2, n_rep=16)
     og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
     g = gpu_grid(api, cfg["sub"], cfg["desc"])
     ot, mol = oracle_side(orc, cfg, og), gpu_side(api, cfg)
     vel = np.zeros_like(cfg["pos"])
-    kw = dict(f_tol=1e-3, restart=1, seed=1002, max_step=0.1)
-    r = run_gpu(api, g, mol, api.make_integrator("fire", 6000, 0.5, **kw), cfg["pos"], vel, fire=np.zeros((24, 4), np.float32), minima_cap=2048)
-    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 6000, 0.5, **kw), cfg["pos"], vel, minima_cap=2048)
+    # config 2's f_tol 1e-3 with dt_max 20 fs: with real masses the 60-atom chain needs 1e4-3e4 steps per minimum (DESIGN.md R13)
+    kw = dict(f_tol=1e-3, dt_max=20.0, restart=1, seed=1002, max_step=0.1)
+    r = run_gpu(api, g, mol, api.make_integrator("fire", 40000, 1.0, **kw), cfg["pos"], vel, fire=np.zeros((16, 4), np.float32), minima_cap=2048)
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 40000, 1.0, **kw), cfg["pos"], vel, minima_cap=2048)
     assert r["n_minima"] > 0 and o["n_minima"] > 0
     key = lambda m: {(int(x[0]), int(x[1])): x for x in m}
     kg, ko = key(r["minima"]), key(o["minima"])
     common = sorted(set(kg) & set(ko))
-    assert len(common) >= 0.5 * min(len(kg), len(ko))
+    assert len(common) >= 0.5 * min(len(kg), len(ko)) and len(common) >= 4
     Eg = np.array([kg[c][3] for c in common]); Eo = np.array([ko[c][3] for c in common])
     xg = np.array([kg[c][4:] for c in common]).reshape(len(common), -1, 3); xo = np.array([ko[c][4:] for c in common]).reshape(len(common), -1, 3)
     same = basin_match(Eg, xg, Eo, xo, cfg["desc"]["Lx"], cfg["desc"]["Ly"])
@@ -340,7 +363,7 @@ def test_fire_restart_basins_config2(api, orc):
     # every recorded GPU minimum really is one: max |F_i| < f_tol when re-evaluated by the oracle
     for c in common[:10]:
         E7, F = orc.forces(og, ot, kg[c][4:].reshape(-1, 3))
-        assert np.sqrt((F ** 2).sum(1)).max() < 2e-3
+        assert np.sqrt((F ** 2).sum(1)).max() < 1.05e-3
 
 
 def test_run_replicas_host_and_determinism(api, cfg1s):
