@@ -159,7 +159,8 @@ typedef struct {
     int restart;              /* FIRE: 0 stop when converged; 1 record the minimum and re-seed from Philox4x32-10(seed, replica, restart#) */
     unsigned long long seed;
     float z_ref, place_z_lo, place_z_hi, place_z_min, clash;   /* restart placement (3, 6, 2 Å above z_ref; clash factor 0.4) */
-    int variant;              /* kernel variant: 0 = default (library's choice), 1 = one thread per atom gathers its 64 nodes, 2 = warp-cooperative row gather */
+    int variant;              /* kernel variant: 0 = default (library's choice), 1 = one thread per atom gathers its 64 nodes, 2 = warp-cooperative row gather every step,
+                                 3 = 2 + the folded stencils cached in shared memory and re-gathered only when an atom changes cell */
 } gridff_integrator;
 
 /* Advance n_rep independent replicas of one molecule for integ->n_steps steps in ONE launch sequence without host

@@ -108,6 +108,18 @@ __device__ __forceinline__ void gather_rows(const GridGeom& g, unsigned base, co
     tile[tile_word(slot, lane + 32)] = fold4(cf, n1);
 }
 
+// the same gather split into its load and its fold + store halves, so that several stencils can be in flight
+__device__ __forceinline__ void load_rows(const GridGeom& g, unsigned base, int lane, float4& n0, float4& n1) {
+    const int k = lane & 3, r0 = lane >> 2;
+    const int rs = g.nzp, ps = g.sy * g.nzp;
+    const float4* p = g.store + base + (r0 >> 2) * ps + (r0 & 3) * rs + k;
+    n0 = __ldg(p); n1 = __ldg(p + 2 * ps);
+}
+__device__ __forceinline__ void store_rows(const float4 cf, const float4 n0, const float4 n1, int lane, int slot, float* tile) {
+    tile[tile_word(slot, lane)] = fold4(cf, n0);
+    tile[tile_word(slot, lane + 32)] = fold4(cf, n1);
+}
+
 // owner-side evaluation from the tile (after __syncwarp)
 __device__ __forceinline__ void interp_tile(const GridGeom& g, const Stencil& s, int slot, const float* tile, float& E, float& Fx, float& Fy, float& Fz) {
     if (s.base == kNoStencil) { E = Fx = Fy = Fz = 0.f; return; }

@@ -161,7 +161,7 @@ def check_energies(eg, eo, tol_rel=2e-5, tol_abs=2e-5):
         assert np.abs(eg[:, c] - eo[:, c]).max() <= tol_abs + tol_rel * scale * 10, (c, np.abs(eg[:, c] - eo[:, c]).max(), scale)
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 @pytest.mark.parametrize("k", [0, 1, 2])
 def test_energy_terms_at_fixed_state(api, orc, k, variant):
     """n_steps = 0: the launch only evaluates the energy terms of the input state (a9)"""
@@ -177,7 +177,7 @@ def test_energy_terms_at_fixed_state(api, orc, k, variant):
     check_energies(r["energy"], o["energy"])
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 @pytest.mark.parametrize("k", [1, 2])
 def test_vv_trajectory_100_steps(api, orc, k, variant):
     """velocity Verlet, dt = 0.5 fs, 300 K start: positions within 1e-3 Å of the fp64 oracle after 100 steps (north_star)"""
@@ -194,6 +194,18 @@ def test_vv_trajectory_100_steps(api, orc, k, variant):
     assert np.abs(r["vel"].astype(np.float64) - o["vel"]).max() <= 1e-4          # Å/fs; thermal speeds are ~1e-2
     assert np.all(r["status"][:, 0] == 100) and np.all(r["status"][:, 1] == 0)
     check_energies(r["energy"], o["energy"], tol_rel=1e-4, tol_abs=2e-4)
+
+
+@pytest.mark.parametrize("k", [1, 2])
+def test_stencil_cache_is_bit_identical(api, k):
+    """variant 3 (folded stencils cached, re-gathered on cell change) computes exactly what variant 2 (gather every step) does"""
+    cfg = small_config(k, n_rep=41)
+    g = gpu_grid(api, cfg["sub"], cfg["desc"])
+    mol = gpu_side(api, cfg)
+    vel = inputs.maxwell_boltzmann(cfg["topo"], 41, 600.0, 17)
+    r2 = run_gpu(api, g, mol, api.make_integrator("vv", 400, 0.5, variant=2), cfg["pos"], vel)
+    r3 = run_gpu(api, g, mol, api.make_integrator("vv", 400, 0.5, variant=3), cfg["pos"], vel)
+    assert np.array_equal(r2["pos"], r3["pos"]) and np.array_equal(r2["vel"], r3["vel"]) and np.array_equal(r2["energy"], r3["energy"])
 
 
 def test_vv_gas_phase_and_launch_split(api, orc):
@@ -239,7 +251,7 @@ def basin_match(Eg, xg, Eo, xo, Lx, Ly):
     return (np.abs(Eg - Eo) < 1e-3) & (rmsd < 0.1)
 
 
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_fire_relaxation_config0(api, orc, variant):
     """config 0 (benzene, 2 Morse channels) on the small slab, 48 replicas.  (a) the config as stated: 1000 FIRE steps, dt0 0.5 fs,
     f_tol 1e-3 — with real masses few replicas converge that fast (DESIGN.md R13), so the final states are compared;
