@@ -61,8 +61,8 @@ __global__ void __launch_bounds__(128) k_eval_brick(GridGeom g, long long n, con
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= n) return;
     int ix, iy, iz; float tx, ty, tz;
-    cell_periodic(pos[3 * p], g.inv_hx_hi, g.inv_hx_lo, g.nx, ix, tx);
-    cell_periodic(pos[3 * p + 1], g.inv_hy_hi, g.inv_hy_lo, g.ny, iy, ty);
+    cell_periodic(pos[3 * p], g.inv_hx_hi, g.inv_hx_lo, g.fnx, g.inv_nx, ix, tx);
+    cell_periodic(pos[3 * p + 1], g.inv_hy_hi, g.inv_hy_lo, g.fny, g.inv_ny, iy, ty);
     float e = 0.f, fx = 0.f, fy = 0.f, fz = 0.f;
     if (cell_z(pos[3 * p + 2], g, iz, tz)) {
         const float4 cf = coef[p];

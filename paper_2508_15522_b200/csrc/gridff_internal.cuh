@@ -24,6 +24,7 @@ struct GridGeom {
     float inv_hx_hi, inv_hx_lo, inv_hy_hi, inv_hy_lo, inv_hz_hi, inv_hz_lo;
     float z0_hi, z0_lo;          // z of node 0 (z_ref + z_lo), split
     float inv_hx, inv_hy, inv_hz;
+    float fnx, inv_nx, fny, inv_ny;   // (float)nx, 1/nx, ...: cell wrap without an integer division
     const float4* store;
 };
 
@@ -61,13 +62,18 @@ __device__ __forceinline__ void bspline_w(float t, float w[4], float d[4]) {
 }
 
 // cell index (wrapped into [0,n)) and fraction along a periodic axis
-__device__ __forceinline__ void cell_periodic(float x, float inv_hi, float inv_lo, int n, int& i, float& t) {
+__device__ __forceinline__ void cell_periodic(float x, float inv_hi, float inv_lo, float fn, float inv_n, int& i, float& t) {
     float fi = floorf(x * inv_hi);
     float tt = fmaf(x, inv_hi, -fi) + x * inv_lo;
     if (tt < 0.0f) { tt += 1.0f; fi -= 1.0f; }
     if (tt >= 1.0f) { tt -= 1.0f; fi += 1.0f; }
-    int ii = (int)fi % n;                 // |fi| < 2^24 for any sane coordinate; NaN -> 0
-    if (ii < 0) ii += n;
+    // fi mod n in floats: fi is an integer with |fi| < 2^24 for any sane coordinate, so fi - q n is exact; the rounded
+    // quotient can be off by one either way
+    float r = fmaf(-floorf(fi * inv_n), fn, fi);
+    if (r < 0.0f) r += fn;
+    if (r >= fn) r -= fn;
+    int ii = (int)r;                      // NaN -> 0
+    ii = min(max(ii, 0), (int)fn - 1);    // and never outside the store, whatever x was
     i = ii; t = tt;
 }
 

@@ -15,8 +15,8 @@ constexpr unsigned kNoStencil = 0xFFFFFFFFu;
 
 __device__ __forceinline__ Stencil locate(const GridGeom& g, float x, float y, float z) {
     Stencil s; int ix, iy, iz;
-    cell_periodic(x, g.inv_hx_hi, g.inv_hx_lo, g.nx, ix, s.tx);
-    cell_periodic(y, g.inv_hy_hi, g.inv_hy_lo, g.ny, iy, s.ty);
+    cell_periodic(x, g.inv_hx_hi, g.inv_hx_lo, g.fnx, g.inv_nx, ix, s.tx);
+    cell_periodic(y, g.inv_hy_hi, g.inv_hy_lo, g.fny, g.inv_ny, iy, s.ty);
     if (cell_z(z, g, iz, s.tz)) s.base = (unsigned)corner_zfast(g, ix, iy, iz);
     else { s.base = kNoStencil; s.tz = 0.f; }
     return s;
