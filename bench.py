@@ -38,11 +38,15 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="gridff", choices=["gridff", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 3])
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--md-steps", type=int, default=0, help="override the config's MD steps per launch (0 = config value)")
     ap.add_argument("--replicas", type=int, default=0, help="override the config's replica count (0 = config value)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--log2-points", type=int, default=26, help="config 4: number of interpolation points = 2^k")
+    ap.add_argument("--order", default="random", choices=["random", "sorted"], help="config 4: point order (sorted = Morton order of the cell)")
+    ap.add_argument("--c4-grid", default="config1", help="config 4: 'config1' (the 113 x 113 x 100 NaCl grid) or NXxNYxNZ synthetic sweep grid")
+    ap.add_argument("--sweep", action="store_true", help="config 4: also time the grid-size x order sweep (32^3 ... 512x512x256)")
     return ap.parse_args()
 
 
@@ -50,7 +54,9 @@ def workload(args):
     cfg = inputs.config(args.config, n_rep=args.replicas or None)
     md = args.md_steps or cfg["integ"]["n_steps"]
     nx, ny, nz = inputs.grid_dims(cfg["desc"])
-    name = {0: "config0: 64 x benzene FIRE", 1: "config1: NaCl(001) 4x4 slab + Coulomb, 4096 x 30-atom aromatic, VV dt 0.5 fs x 10000",
+    name = {0: "config0: NaCl(001) 4x4 slab, 2 channels, 64 x benzene, FIRE x 1000",
+            2: "config2: config1 grid, 16384 x 60-atom flexible chain, FIRE to 1e-3 eV/A (cap 20000) + Philox restart",
+            1: "config1: NaCl(001) 4x4 slab + Coulomb, 4096 x 30-atom aromatic, VV dt 0.5 fs x 10000",
             3: "config3: 40x40 Å slab, 400x400x150x4 grid (384 MB), 8192 x 30-atom aromatic, VV x 5000"}[args.config]
     return cfg, md, (nx, ny, nz), name
 
@@ -140,7 +146,7 @@ class ClockSampler:
 def run_gridff(args):
     import torch
     import torch.distributed as dist
-    from paper_2508_15522_b200 import api            # raises if the CUDA library is missing: there is no fallback
+    from paper_2508_15522_b200 import api, shard     # api raises if the CUDA library is missing: there is no fallback
 
     world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
@@ -151,12 +157,17 @@ def run_gridff(args):
     cfg, md, dims, name = workload(args)
     # replicas only: every rank runs its own batch of the same size with its own seed; no data-path collective
     if world > 1:
-        cfg["pos"] = inputs.place_replicas(cfg["topo"], cfg["n_rep"], cfg["desc"]["Lx"], cfg["desc"]["Ly"], 0.0, cfg["seed"] + 10 + 1000 * rank)
+        cfg["pos"] = inputs.place_replicas(cfg["topo"], cfg["n_rep"], cfg["desc"]["Lx"], cfg["desc"]["Ly"], 0.0, shard.rank_seed(cfg["seed"], rank, 10),
+                                           twist=(args.config == 2))
     d, topo, sub = cfg["desc"], cfg["topo"], cfg["sub"]
     n_rep, n_at = cfg["n_rep"], int(topo["n_atoms"])
     desc = api.make_desc(d["Lx"], d["Ly"], d["z_ref"], d["z_lo"], d["z_hi"], d["spacing"], d["alpha"], d["channels"], r_cut=d["r_cut"], l2_persist=1)
     kind = cfg["integ"]["kind"]
-    integ = api.make_integrator(kind, md, cfg["integ"]["dt"], f_tol=cfg["integ"].get("f_tol", 1e-3), variant=args.variant)
+    restart = int(cfg["integ"].get("restart", 0))
+    ikw = dict(f_tol=cfg["integ"].get("f_tol", 1e-3), variant=args.variant)
+    if restart:          # config 2: relax, record the minimum, re-seed from Philox (R13, R17); dt_max / max_step as in the parity test
+        ikw.update(restart=1, seed=shard.rank_seed(cfg["integ"]["seed"], rank), dt_max=20.0, max_step=0.1)
+    integ = api.make_integrator(kind, md, cfg["integ"]["dt"], **ikw)
     mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
     sub_pos = np.ascontiguousarray(sub["pos"], np.float64); sub_e = np.ascontiguousarray(sub["e"], np.float64)
     sub_R = np.ascontiguousarray(sub["R"], np.float64); sub_q = np.ascontiguousarray(sub["q"], np.float64)
@@ -166,6 +177,9 @@ def run_gridff(args):
     d_pos, d_vel = torch.empty_like(pos0), torch.empty_like(vel0)
     d_energy = torch.empty((n_rep, 8), device="cuda"); d_status = torch.empty((n_rep, 2), dtype=torch.int32, device="cuda")
     d_fire = torch.zeros((n_rep, 4), device="cuda")
+    minima_cap = 8 * n_rep if restart else 0
+    d_minima = torch.zeros((minima_cap, 4 + 3 * n_at), device="cuda") if restart else None
+    d_n_minima = torch.zeros(1, dtype=torch.int32, device="cuda") if restart else None
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")          # > 126 MB L2
     stream = torch.cuda.current_stream()
     sptr = C.c_void_p(stream.cuda_stream)
@@ -181,12 +195,14 @@ def run_gridff(args):
     def one_step():
         """-> (ms whole step, ms of the fused replica kernel alone)"""
         d_pos.copy_(pos0); d_vel.copy_(vel0); d_fire.zero_()
+        if restart:
+            d_n_minima.zero_()
         flush.fill_(1)                                    # L2 flush between timed iterations
         e0, e1, e2 = ev(), ev(), ev()
         e0.record(stream)
         g = build()
         e1.record(stream)
-        api.gridff_run_replicas(g, mol, integ, d_pos, d_vel, d_fire=d_fire, d_energy=d_energy, d_status=d_status)
+        api.gridff_run_replicas(g, mol, integ, d_pos, d_vel, d_fire=d_fire, d_energy=d_energy, d_status=d_status, d_minima=d_minima, d_n_minima=d_n_minima)
         e2.record(stream)
         e2.synchronize()
         return e0.elapsed_time(e2), e1.elapsed_time(e2), g
@@ -208,13 +224,24 @@ def run_gridff(args):
     barrier()
     launches = api.gridff_launch_count() - l0
     clocks = sampler.stop() if sampler else None
-    total_ms = float(np.sum(t_step))
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(float(np.sum(t_step)), "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * n_rep * md / (ms_per_step * 1e-3)
+    # units one step processed on this rank: VV runs md steps per replica; FIRE counts the steps really taken (converged replicas stop)
+    units = n_rep * md if kind == "vv" else int(d_status[:, 0].sum().item())
+    units_all = float(shard.sum_over_ranks(np.array([float(units)]), "cuda")[0])
+    value = units_all / (ms_per_step * 1e-3)
+    sampling = None
+    if restart:
+        nm = int(d_n_minima.item())
+        e_min = d_minima[:min(nm, minima_cap), 3].cpu().numpy()
+        nm_all = float(shard.sum_over_ranks(np.array([float(nm)]), "cuda")[0])
+        lo = float(np.floor(e_min.min() * 10) / 10) if len(e_min) else 0.0
+        lo = -shard.max_over_ranks(-lo, "cuda"); hi = lo + 4.0
+        hist = shard.sum_over_ranks(shard.basin_histogram(e_min, lo, hi, 0.01), "cuda")
+        nzb = np.nonzero(hist)[0]
+        sampling = {"relaxed_configs_per_s": nm_all / (ms_per_step * 1e-3), "minima_per_step": nm_all, "minima_cap_per_gpu": minima_cap,
+                    "basin_energy_histogram": {"bin_eV": 0.01, "e_lo_eV": lo, "first_bin": int(nzb[0]) if len(nzb) else 0,
+                                               "counts": hist[nzb[0]:nzb[-1] + 1].tolist() if len(nzb) else []}}
     assert bool(torch.isfinite(d_pos).all()), "non-finite positions after the timed run"
 
     # ---- end to end through the public host-buffer API: pinned host inputs -> device -> pinned host results, every step
@@ -232,12 +259,9 @@ def run_gridff(args):
         dt_ms = (time.perf_counter() - t0) * 1e3
         if it >= 2:
             e2e_ms.append(dt_ms)
-    e2e_total = float(np.sum(e2e_ms))
-    if world > 1:
-        t = torch.tensor([e2e_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_total = float(t.item())
-    e2e_value = world * n_rep * md / (e2e_total / args.steps * 1e-3)
+    e2e_total = shard.max_over_ranks(float(np.sum(e2e_ms)), "cuda")
+    e2e_units = n_rep * md if kind == "vv" else int(hs[:, 0].sum().item())
+    e2e_value = float(shard.sum_over_ranks(np.array([float(e2e_units)]), "cuda")[0]) / (e2e_total / args.steps * 1e-3)
     h2d = 2 * n_rep * n_at * 12 + sub_pos.nbytes + sub_e.nbytes + sub_R.nbytes + sub_q.nbytes
     d2h = 2 * n_rep * n_at * 12 + n_rep * 32 + n_rep * 8
 
@@ -247,8 +271,9 @@ def run_gridff(args):
         return
 
     # ---- roofline of the dominant kernel (the fused replica kernel): algorithmic gather bytes / measured duration
-    force_evals = md + 2 if kind == "vv" else md + 1                     # initial + per step + final energy pass
-    bytes_per_launch = float(n_rep) * n_at * force_evals * BYTES_PER_EVAL
+    # force evaluations per launch: VV = initial + per step + final energy pass; FIRE = one per step taken + final energy pass
+    evals_per_launch = float(n_rep) * n_at * (md + 2) if kind == "vv" else float(units + n_rep) * n_at
+    bytes_per_launch = evals_per_launch * BYTES_PER_EVAL
     kern_ms = float(np.mean(t_kern))
     achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
     peaks = {}
@@ -258,7 +283,7 @@ def run_gridff(args):
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0)); hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6.65 TB/s (B200_PROFILING.md)"
     # L2 read bandwidth measured live with the library's probe over a buffer the size of the coefficient store (stays in L2)
-    probe = torch.empty(min(sb, 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)
+    probe = torch.empty(min(max(sb, 16 << 20), 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)
     l2 = {}
     for mode, key in ((0, "stream"), (1, "rows64")):
         api.gridff_probe_read(probe, iters=20, mode=mode); torch.cuda.synchronize()
@@ -278,7 +303,7 @@ def run_gridff(args):
         pass
     roofline = {"bound": bound, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
                 "kernel": "k_replicas (fused grid + intramolecular + integrator)", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
-                "bytes_per_eval": BYTES_PER_EVAL, "evals_per_launch": n_rep * n_at * force_evals,
+                "bytes_per_eval": BYTES_PER_EVAL, "evals_per_launch": evals_per_launch,
                 "peak_source": ("L2 read bandwidth measured in this run by gridff_probe_read (coalesced 16 B loads over a %d MB buffer)" % (probe.numel() >> 20))
                 if store_fits_l2 else hbm_src,
                 "l2_probe_gbs": l2, "hbm_peak_gbs": hbm_peak, "frac_of_hbm_peak": achieved / hbm_peak}
@@ -286,7 +311,7 @@ def run_gridff(args):
     cpu = None
     if not args.no_cpu_baseline:
         tb, tps, cores, n, ss = oracle_sample(cfg, md)
-        tot = n_rep * md
+        tot = units
         cpu = {"value": tot / (tb + tot * tps), "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "full fp64 grid build (a1-a3, %.1f s) + %d replicas x %d steps (%.3g s per replica-step), extrapolated to %d x %d" % (tb, n, ss, tps, n_rep, md),
                "replica_steps_per_s_run_only": 1.0 / tps}
@@ -297,7 +322,7 @@ def run_gridff(args):
         "config": {"workload": name, "grid": list(dims), "channels": len(d["channels"]), "store_bytes": sb, "n_replicas_per_gpu": n_rep,
                    "md_steps_per_step": md, "atoms": n_at, "integrator": kind, "variant": args.variant, "parallelism": "replicas only (no collective)",
                    "l2_flush_between_steps": True, "step": "gridff_build_grid + gridff_run_replicas"},
-        "atom_grid_evals_per_s": value * n_at,
+        "atom_grid_evals_per_s": value * n_at, "sampling": sampling,
         "ms_build_grid": ms_per_step - kern_ms,
         "clocks": clocks, "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}))
@@ -305,9 +330,249 @@ def run_gridff(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------------------------ config 4
+# Bare interpolation microbenchmark (BASELINE.json configs[4]): 2^26 uniformly random points in the config-1 grid volume, 3-channel E
+# and analytic gradient per point; optional sweep over grid sizes 32^3 ... 512 x 512 x 256, random vs Morton-sorted point order.
+
+C4_METRIC, C4_UNIT = "atom_grid_evals_per_s", "evals/s"
+C4_SWEEP = [(32, 32, 32), (64, 64, 64), (128, 128, 128), (256, 256, 256), (512, 512, 256)]
+C4_IO_BYTES = 12 + 16 + 4 + 12            # pos + coef in, E + F out per point (streamed through HBM whatever the grid size)
+
+
+def c4_grid_spec(args):
+    """-> (name, dims, desc dict, substrate or None)"""
+    if args.c4_grid == "config1":
+        cfg = inputs.config(1, n_rep=1)
+        return "config1 grid (NaCl(001) 4x4 slab, Pauli + London + Coulomb)", inputs.grid_dims(cfg["desc"]), cfg["desc"], cfg["sub"]
+    nx, ny, nz = (int(v) for v in args.c4_grid.lower().split("x"))
+    return "synthetic %dx%dx%d" % (nx, ny, nz), (nx, ny, nz), c4_synth_desc(nx, ny, nz), None
+
+
+def c4_synth_desc(nx, ny, nz, h=0.1):
+    return inputs.grid_desc(nx * h, ny * h, 0.0, 1.5, 1.5 + nz * h, h, 1.6, [inputs.PAULI, inputs.LONDON, inputs.COULOMB])
+
+
+def c4_valid_z(desc, nz):
+    z0 = desc["z_ref"] + desc["z_lo"]
+    return z0 + desc["spacing"], z0 + (nz - 2) * desc["spacing"] - 1e-3          # DESIGN.md R5
+
+
+def run_eval_reference(args):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import gridff_oracle as orc
+    name, dims, d, sub = c4_grid_spec(args)
+    nx, ny, nz = dims; z0 = d["z_ref"] + d["z_lo"]
+    if sub is not None:
+        samples = orc.sample_grid(sub, d["alpha"], d["Lx"], d["Ly"], d["r_cut"], nx, ny, nz, z0, d["spacing"], d["channels"])
+    else:
+        samples = inputs.c4_samples(nx, ny, nz).astype(np.float64)
+    og = orc.OracleGrid(orc.prefilter(samples, (1, 1, 0)), d["Lx"], d["Ly"], z0, d["spacing"])
+    n_s = 1 << 22
+    zl, zh = c4_valid_z(d, nz)
+    pos, coef = inputs.c4_points(n_s, d["Lx"], d["Ly"], zl, zh)
+    ts = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter(); orc.interp(og, pos, coef); t = time.perf_counter() - t0
+        if it >= args.warmup:
+            ts.append(t)
+    val = n_s / float(np.mean(ts)); n = 1 << args.log2_points
+    sample = "2^22 of the 2^%d points per step (grid resident, fp64 coefficients)" % args.log2_points
+    print(json.dumps({
+        "impl": "reference", "metric": C4_METRIC, "value": val, "unit": C4_UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": n / val * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config4: 2^%d random points, %s" % (args.log2_points, name), "grid": list(dims), "order": "random"},
+        "cpu_baseline": {"value": val, "unit": C4_UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": C4_UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def run_eval(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2508_15522_b200 import api, shard
+
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    stream = torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0)); hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6.65 TB/s (B200_PROFILING.md)"
+
+    def make_grid(desc, dims, sub):
+        gd = api.make_desc(desc["Lx"], desc["Ly"], desc["z_ref"], desc["z_lo"], desc["z_hi"], desc["spacing"], desc["alpha"], desc["channels"],
+                           r_cut=desc["r_cut"], l2_persist=1)
+        if sub is not None:
+            return api.gridff_build_grid(gd, sub["pos"], sub["e"], sub["R"], sub["q"])
+        smp = inputs.c4_samples(*dims, xp=torch, device="cuda")
+        g = api.gridff_grid_from_samples(gd, smp)
+        del smp
+        return g
+
+    def make_points(desc, dims, n, seed):
+        zl, zh = c4_valid_z(desc, dims[2])
+        pos, coef = inputs.c4_points(n, desc["Lx"], desc["Ly"], zl, zh, seed=seed)
+        return pos, coef
+
+    def l2_probe(nbytes):
+        probe = torch.empty(min(max(nbytes, 16 << 20), 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)     # >= 16 MB: a smaller buffer cannot occupy every SM
+        out = {}
+        for mode, key in ((0, "stream"), (1, "rows64")):
+            api.gridff_probe_read(probe, iters=20, mode=mode); torch.cuda.synchronize()
+            best = 0.0
+            for _ in range(5):
+                a, b = ev(), ev()
+                a.record(stream); api.gridff_probe_read(probe, iters=100, mode=mode); b.record(stream); b.synchronize()
+                best = max(best, probe.numel() * 100 / (a.elapsed_time(b) * 1e-3) / 1e9)
+            out[key] = best
+        return out
+
+    def time_eval(g, d_pos, d_coef, d_E, d_F, reps, warm):
+        ts = []
+        for it in range(warm + reps):
+            flush.fill_(1)
+            a, b = ev(), ev()
+            a.record(stream); api.gridff_eval(g, d_pos, d_coef, d_E=d_E, d_F=d_F); b.record(stream); b.synchronize()
+            if it >= warm:
+                ts.append(a.elapsed_time(b))
+        return ts
+
+    name, dims, desc, sub = c4_grid_spec(args)
+    n = 1 << args.log2_points
+    g = make_grid(desc, dims, sub)
+    sb = g.store.numel()
+    pos, coef = make_points(desc, dims, n, shard.rank_seed(1004, rank))
+    d_pos, d_coef = torch.from_numpy(pos).cuda(), torch.from_numpy(coef).cuda()
+    z0 = desc["z_ref"] + desc["z_lo"]
+    if args.order == "sorted":
+        perm = inputs.morton_order(d_pos, desc["Lx"], desc["Ly"], z0, dims[0], dims[1], desc["spacing"], xp=torch)
+        d_pos, d_coef = d_pos[perm].contiguous(), d_coef[perm].contiguous()
+        pos, coef = d_pos.cpu().numpy(), d_coef.cpu().numpy()
+        del perm
+    d_E = torch.empty(n, device="cuda"); d_F = torch.empty((n, 3), device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    time_eval(g, d_pos, d_coef, d_E, d_F, 0, max(args.warmup, 3))
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = api.gridff_launch_count()
+    ts = time_eval(g, d_pos, d_coef, d_E, d_F, args.steps, 0)
+    barrier()
+    launches = api.gridff_launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    total_ms = shard.max_over_ranks(float(np.sum(ts)), "cuda")
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+    assert bool(torch.isfinite(d_E).all()), "non-finite energies after the timed run"
+
+    # ---- end to end: pinned host points -> device -> pinned host E, F through gridff_eval_host, every step
+    hp, hc = torch.from_numpy(pos).pin_memory(), torch.from_numpy(coef).pin_memory()
+    hE, hF = torch.empty(n).pin_memory(), torch.empty((n, 3)).pin_memory()
+    d_work = torch.empty(api.gridff_eval_work_bytes(n), dtype=torch.uint8, device="cuda")
+    e2e_ms = []
+    for it in range(2 + args.steps):
+        flush.fill_(1); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        api.gridff_eval_host(g, hp, hc, hE, hF, d_work=d_work)           # synchronises
+        if it >= 2:
+            e2e_ms.append((time.perf_counter() - t0) * 1e3)
+    e2e_total = shard.max_over_ranks(float(np.sum(e2e_ms)), "cuda")
+    e2e_value = world * n / (e2e_total / args.steps * 1e-3)
+    assert float((hE - d_E.cpu()).abs().max()) == 0.0, "host path and device path disagree"
+    del hp, hc, hE, hF, d_work
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    def roof(store_bytes, n_pts, ms, l2):
+        fits = store_bytes < (100 << 20)
+        ach = n_pts * float(BYTES_PER_EVAL) / (ms * 1e-3) / 1e9
+        peak = l2["stream"] if fits else hbm_peak
+        return fits, ach, peak
+
+    l2 = l2_probe(sb)
+    kern_ms = float(np.mean(ts))
+    fits, ach, peak = roof(sb, n, kern_ms, l2)
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get("config4")
+    except Exception:
+        pass
+    roofline = {"bound": "l2" if fits else "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
+                "kernel": "k_eval_coop (warp-cooperative tricubic gather)", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
+                "bytes_per_eval": BYTES_PER_EVAL, "evals_per_launch": n, "io_bytes_per_eval_hbm": C4_IO_BYTES,
+                "io_stream_gbs": n * float(C4_IO_BYTES) / (kern_ms * 1e-3) / 1e9,
+                "peak_source": "L2 read bandwidth measured in this run by gridff_probe_read" if fits else hbm_src,
+                "l2_probe_gbs": l2, "hbm_peak_gbs": hbm_peak, "frac_of_hbm_peak": ach / hbm_peak}
+
+    sweep = None
+    if args.sweep:
+        sweep = []
+        del d_pos, d_coef
+        specs = [("config1", dims, desc, sub)] + [("%dx%dx%d" % s_, s_, c4_synth_desc(*s_), None) for s_ in C4_SWEEP]
+        for gname, gdims, gdesc, gsub in specs:
+            gg = make_grid(gdesc, gdims, gsub)
+            gsb = gg.store.numel()
+            gl2 = l2_probe(gsb) if gsb < (100 << 20) else l2
+            p_, c_ = make_points(gdesc, gdims, n, 1004)
+            dp, dc = torch.from_numpy(p_).cuda(), torch.from_numpy(c_).cuda()
+            for order in ("random", "sorted"):
+                if order == "sorted":
+                    perm = inputs.morton_order(dp, gdesc["Lx"], gdesc["Ly"], gdesc["z_ref"] + gdesc["z_lo"], gdims[0], gdims[1], gdesc["spacing"], xp=torch)
+                    dp, dc = dp[perm].contiguous(), dc[perm].contiguous()
+                    del perm
+                t = float(np.mean(time_eval(gg, dp, dc, d_E, d_F, 3, 2)))
+                f_, a_, pk = roof(gsb, n, t, gl2)
+                sweep.append({"grid": gname, "store_MB": round(gsb / 1e6, 1), "order": order, "ms": t, "evals_per_s": n / (t * 1e-3),
+                              "gather_GBs": a_, "bound": "l2" if f_ else "hbm", "peak_GBs": pk, "frac": a_ / pk})
+                sys.stderr.write("sweep %-12s %7.1f MB %-6s %8.3f ms  %.3e evals/s  %8.1f GB/s  %.3f of %s\n"
+                                 % (gname, gsb / 1e6, order, t, n / (t * 1e-3), a_, a_ / pk, "l2" if f_ else "hbm"))
+            del dp, dc
+            gg.free()
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import gridff_oracle as orc
+        nx, ny, nz = dims
+        if sub is not None:
+            samples = orc.sample_grid(sub, desc["alpha"], desc["Lx"], desc["Ly"], desc["r_cut"], nx, ny, nz, z0, desc["spacing"], desc["channels"])
+        else:
+            samples = inputs.c4_samples(nx, ny, nz).astype(np.float64)
+        og = orc.OracleGrid(orc.prefilter(samples, (1, 1, 0)), desc["Lx"], desc["Ly"], z0, desc["spacing"])
+        n_s = min(n, 1 << 22)
+        orc.interp(og, pos[:1 << 16], coef[:1 << 16])
+        t0 = time.perf_counter(); orc.interp(og, pos[:n_s], coef[:n_s]); t = time.perf_counter() - t0
+        cpu = {"value": n_s / t, "unit": C4_UNIT, "cores": orc.num_threads(), "kind": "oracle",
+               "sample": "the first 2^%d of the 2^%d points (%.2f s), grid resident, fp64" % (int(np.log2(n_s)), args.log2_points, t)}
+
+    print(json.dumps({
+        "metric": C4_METRIC, "value": value, "unit": C4_UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config4: 2^%d uniformly random points, %s, 3-channel E + analytic gradient" % (args.log2_points, name),
+                   "grid": list(dims), "store_bytes": sb, "points_per_gpu": n, "order": args.order, "parallelism": "points only (no collective)",
+                   "l2_flush_between_steps": True, "step": "gridff_eval over all points (grid built before the timed region)"},
+        "clocks": clocks, "e2e": {"value": e2e_value, "unit": C4_UNIT, "h2d_bytes_per_step": n * 28, "d2h_bytes_per_step": n * 16},
+        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "sweep": sweep}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
-        run_reference(a)
+        run_eval_reference(a) if a.config == 4 else run_reference(a)
     else:
-        run_gridff(a)
+        run_eval(a) if a.config == 4 else run_gridff(a)

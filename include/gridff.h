@@ -150,7 +150,7 @@ int gridff_create_molecule(const gridff_topology* topo, void* d_buf, size_t buf_
 int gridff_free_molecule(gridff_molecule* mol);
 
 typedef struct {
-    int kind;                 /* 0 velocity Verlet, 1 FIRE (ref 72) */
+    int kind;                 /* 0 velocity Verlet, 1 FIRE (ref 72), 2 Langevin dynamics (BAOAB, R18) */
     int n_steps;              /* steps per launch (FIRE: upper bound) */
     float dt;                 /* fs (FIRE: initial dt) */
     float f_tol;              /* FIRE stops when max_i |F_i| < f_tol, eV/Å */
@@ -161,6 +161,16 @@ typedef struct {
     float z_ref, place_z_lo, place_z_hi, place_z_min, clash;   /* restart placement (3, 6, 2 Å above z_ref; clash factor 0.4) */
     int variant;              /* kernel variant: 0 = default (library's choice), 1 = one thread per atom gathers its 64 nodes, 2 = warp-cooperative row gather every step,
                                  3 = 2 + the folded stencils cached in shared memory and re-gathered only when an atom changes cell */
+    /* SURVEY.md §8(f) rows 1-2 (0 / unset = off) */
+    float temperature;        /* K, kind 2 */
+    float gamma;              /* friction 1/fs, kind 2: per step  B: v += dt/2 a;  A: x += dt/2 v;  O: v = c1 v + c2 sqrt(kT/m) xi;  A;  F(x);  B,
+                                 c1 = exp(-gamma dt), c2 = sqrt(1 - c1^2); xi = Box-Muller normals from Philox4x32-10 with counter
+                                 (step0 + step, atom, 'Lang', replica), key = seed, u = ((x >> 9) + 1/2) 2^-23 */
+    unsigned step0;           /* kind 2: index of this launch's first step in the noise stream (1 x N == k x N/k launches) */
+    int n_scan;               /* gridff_run_scan only: number of scan points */
+    unsigned long long fixed_mask;   /* bit i: atom i is held (the restrained atom of PAPER.md:L178, L184): it feels no force, has no velocity and takes
+                                        no part in the convergence test; only a scan moves it */
+    float scan_dx[3];         /* gridff_run_scan: displacement of the held atoms per scan point, Å */
 } gridff_integrator;
 
 /* Advance n_rep independent replicas of one molecule for integ->n_steps steps in ONE launch sequence without host
@@ -175,6 +185,16 @@ typedef struct {
 int gridff_run_replicas(const gridff_grid* grid, const gridff_molecule* mol, const gridff_integrator* integ, int n_rep,
                         float* d_pos, float* d_vel, float* d_fire, float* d_energy, int* d_status,
                         float* d_minima, int minima_cap, int* d_n_minima, void* cuda_stream);
+
+/* Driven scan ("restrained the position of one atom ... displaced the z-component ... by 0.1 Å ... let the position of
+ * the other atoms relax"; L184 dragging): for each of integ->n_scan points, every replica moves its held atoms (fixed_mask) by
+ * scan_dx, then relaxes the others with FIRE (fresh scalars, v = 0) until max_i |F_i| < f_tol or n_steps iterations, all inside
+ * one launch.  integ->kind must be 1, restart 0.
+ *   d_scan  [n_rep][n_scan][4]  out: {E_total (eV), FIRE iterations, converged 0/1, max_i |F_i| over the free atoms} per point
+ *   d_pos / d_vel in/out as in gridff_run_replicas; d_energy / d_status (may be NULL) describe the last point
+ *   (status = {total iterations, points converged}).                                                                 */
+int gridff_run_scan(const gridff_grid* grid, const gridff_molecule* mol, const gridff_integrator* integ, int n_rep,
+                    float* d_pos, float* d_vel, float* d_energy, int* d_status, float* d_scan, void* cuda_stream);
 
 /* Same through HOST buffers (pinned or pageable): copies pos/vel(/fire) to d_work, runs, copies pos/vel/fire/energy/
  * status back, synchronises the stream.  d_work needs gridff_run_work_bytes(mol, n_rep) bytes. */

@@ -22,6 +22,10 @@
  *   FIRE             quadratic-bowl minimum, launch-split invariance          pinned
  *   Philox4x32-10    brute-force big-integer restatement in Python            pinned
  *   restart geometry bond lengths/angles invariant under torsion moves        pinned
+ *   Langevin (BAOAB) gamma = 0 -> velocity Verlet, exact OU decay and equilibrium
+ *                    variance of free particles, equipartition, normal moments  pinned
+ *   held atoms/scan  one-atom scan = the interpolated potential itself;
+ *                    held atoms never move; relaxed E <= unrelaxed E            pinned
  *   basin assignment parity unpinned (only oracle-vs-GPU agreement exists)
  */
 #include <math.h>
@@ -513,7 +517,7 @@ static double rng_uniform(orc_rng* g) {
 }
 
 typedef struct {
-    int kind;               /* 0 velocity Verlet, 1 FIRE */
+    int kind;               /* 0 velocity Verlet, 1 FIRE, 2 Langevin (BAOAB) */
     int n_steps; double dt; /* fs */
     double f_tol;           /* eV/Å: FIRE stops when max_i |F_i| < f_tol */
     double dt_max, f_inc, f_dec, a_start, f_a; int n_min;
@@ -523,6 +527,13 @@ typedef struct {
     double place_z_lo, place_z_hi, place_z_min;  /* centroid height range, lowest-atom floor (3, 6, 2 Å) */
     double clash;           /* reject a conformation with a non-excluded pair closer than clash*(R_i+R_j) */
     double max_step;        /* FIRE: cap on the largest atomic displacement per step, Å (0 = none); R13 */
+    /* SURVEY.md §8(f) rows 1-2 */
+    double temperature;     /* K, Langevin (kind 2; "1000 steps of Langevin molecular dynamics at ... 300 K") */
+    double gamma;           /* friction, 1/fs (kind 2) */
+    uint32_t step0;         /* index of the first step of this call in the noise stream (kind 2): 1 x N == k x N/k */
+    int n_scan;             /* kind 1: > 0 = driven scan: n_scan times {move the held atoms by scan_dx; relax} */
+    uint64_t fixed_mask;    /* bit i: atom i is held (restrained atom of PAPER.md:L178): no force, no velocity, moved only by the scan */
+    double scan_dx[3];      /* Å per scan point */
 } orc_integrator;
 
 /* New conformation for (replica, restart#): template -> random dihedral about every rotatable bond ->
@@ -583,6 +594,29 @@ int orc_restart_conformation(const orc_topology* T, const orc_integrator* I, dou
     return 15;
 }
 
+/* Three standard normals for (replica, step, atom) of the Langevin thermostat (R18): one Philox4x32-10 block with
+ * counter (step, atom, 'Lang', replica) and key = seed; u_k = ((x_k >> 9) + 1/2) 2^-23 in (0,1) (23 random bits: exactly
+ * representable in fp32 and fp64 alike); Box-Muller:
+ * xi_0 = sqrt(-2 ln u_0) cos 2 pi u_1, xi_1 = sqrt(-2 ln u_0) sin 2 pi u_1, xi_2 = sqrt(-2 ln u_2) cos 2 pi u_3. */
+#define ORC_KB 8.617333262e-5       /* eV/K */
+void orc_langevin_normals(uint64_t seed, uint32_t replica, uint32_t step, uint32_t atom, double xi[3]) {
+    uint32_t ctr[4] = {step, atom, 0x4C616E67u, replica}, key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)}, o[4];
+    orc_philox4x32_10(ctr, key, o);
+    double u[4];
+    for (int k = 0; k < 4; ++k) u[k] = ((double)(o[k] >> 9) + 0.5) * (1.0 / 8388608.0);
+    double r0 = sqrt(-2.0 * log(u[0])), r1 = sqrt(-2.0 * log(u[2]));
+    xi[0] = r0 * cos(2.0 * ORC_PI * u[1]);
+    xi[1] = r0 * sin(2.0 * ORC_PI * u[1]);
+    xi[2] = r1 * cos(2.0 * ORC_PI * u[3]);
+}
+
+/* forces with the held atoms' components removed (a held atom takes no part in the dynamics or in the convergence test) */
+static void forces_free(const orc_grid* g, const orc_topology* T, const orc_integrator* I, const double* x, double* F, double* E7) {
+    orc_forces(g, T, x, F, E7);
+    for (int i = 0; i < T->n_atoms; ++i)
+        if ((I->fixed_mask >> i) & 1ull) F[3 * i] = F[3 * i + 1] = F[3 * i + 2] = 0.0;
+}
+
 /* ------------------------------------------------------------------ */
 /* 7. Integrators (steps a7, a8) and outputs (a9)                      */
 /* ------------------------------------------------------------------ */
@@ -602,7 +636,7 @@ static double kinetic(const orc_topology* T, const double* vel) {
  * [n_rep][n_steps+1] total energy after every force evaluation (velocity Verlet only).            */
 void orc_run_replicas(const orc_grid* g, const orc_topology* T, const orc_integrator* I, int n_rep,
                       double* pos, double* vel, double* fire, double* energy, int* status,
-                      double* minima, long minima_cap, long* n_minima, double* e_trace) {
+                      double* minima, long minima_cap, long* n_minima, double* e_trace, double* scan_out) {
     int n = T->n_atoms;
     long nmin = 0;
 #pragma omp parallel for schedule(dynamic, 1)
@@ -612,16 +646,95 @@ void orc_run_replicas(const orc_grid* g, const orc_topology* T, const orc_integr
         double* F = (double*)malloc(sizeof(double) * 3 * (size_t)n);
         double E7[7];
         int steps = 0, flag = 0;
-        if (I->kind == 0) {
+        for (int i = 0; i < n; ++i) if ((I->fixed_mask >> i) & 1ull) v[3 * i] = v[3 * i + 1] = v[3 * i + 2] = 0.0;
+        if (I->kind == 2) {
+            /* Langevin dynamics, BAOAB splitting (Leimkuhler & Matthews 2013; R18):
+             *   B: v += dt/2 a(x);  A: x += dt/2 v;  O: v <- c1 v + c2 sqrt(kT/m) xi;  A: x += dt/2 v;  F(x);  B: v += dt/2 a
+             *   c1 = exp(-gamma dt), c2 = sqrt(1 - c1^2); the O step is the exact Ornstein-Uhlenbeck solution. */
+            const double c1 = exp(-I->gamma * I->dt), c2 = sqrt(1.0 - c1 * c1), kT = ORC_KB * I->temperature;
+            forces_free(g, T, I, x, F, E7);
+            for (int s = 0; s < I->n_steps; ++s) {
+                for (int i = 0; i < n; ++i) {
+                    if ((I->fixed_mask >> i) & 1ull) continue;
+                    double xi[3]; orc_langevin_normals(I->seed, (uint32_t)r, I->step0 + (uint32_t)s, (uint32_t)i, xi);
+                    const double sig = sqrt(kT / T->mass[i] * ORC_ACC);
+                    for (int c = 0; c < 3; ++c) {
+                        v[3 * i + c] += 0.5 * I->dt * F[3 * i + c] / T->mass[i] * ORC_ACC;
+                        x[3 * i + c] += 0.5 * I->dt * v[3 * i + c];
+                        v[3 * i + c] = c1 * v[3 * i + c] + c2 * sig * xi[c];
+                        x[3 * i + c] += 0.5 * I->dt * v[3 * i + c];
+                    }
+                }
+                forces_free(g, T, I, x, F, E7);
+                for (int i = 0; i < n; ++i) for (int c = 0; c < 3; ++c)
+                    v[3 * i + c] += 0.5 * I->dt * F[3 * i + c] / T->mass[i] * ORC_ACC;
+                ++steps;
+            }
+        } else if (I->kind == 1 && I->n_scan > 0) {
+            /* driven scan (PAPER.md:L178 lift, L184 drag): move the held atoms by scan_dx, relax the others with FIRE (fresh scalars,
+             * v = 0) until max |F_i| < f_tol or n_steps iterations, record {E_total, iterations, converged, max |F_i|}; repeat. */
+            for (int sc = 0; sc < I->n_scan; ++sc) {
+                for (int i = 0; i < n; ++i) if ((I->fixed_mask >> i) & 1ull) for (int c = 0; c < 3; ++c) x[3 * i + c] += I->scan_dx[c];
+                for (int i = 0; i < 3 * n; ++i) v[i] = 0;
+                double dt = I->dt, a = I->a_start; int npos = 0, it = 0, conv = 0;
+                for (it = 0; it < I->n_steps; ++it) {
+                    forces_free(g, T, I, x, F, E7);
+                    double fmax2 = 0;
+                    for (int i = 0; i < n; ++i) {
+                        double f2 = F[3 * i] * F[3 * i] + F[3 * i + 1] * F[3 * i + 1] + F[3 * i + 2] * F[3 * i + 2];
+                        if (f2 > fmax2) fmax2 = f2;
+                    }
+                    if (fmax2 < I->f_tol * I->f_tol) { conv = 1; break; }
+                    double P = 0, vv = 0, ff = 0;
+                    for (int i = 0; i < 3 * n; ++i) { P += F[i] * v[i]; vv += v[i] * v[i]; ff += F[i] * F[i]; }
+                    if (P > 0) {
+                        double sc2 = a * sqrt(vv) / sqrt(ff);
+                        for (int i = 0; i < 3 * n; ++i) v[i] = (1.0 - a) * v[i] + sc2 * F[i];
+                        ++npos;
+                        if (npos > I->n_min) { dt = fmin(dt * I->f_inc, I->dt_max); a *= I->f_a; }
+                    } else {
+                        for (int i = 0; i < 3 * n; ++i) v[i] = 0;
+                        dt *= I->f_dec; a = I->a_start; npos = 0;
+                    }
+                    for (int i = 0; i < n; ++i) for (int c = 0; c < 3; ++c)
+                        v[3 * i + c] += dt * F[3 * i + c] / T->mass[i] * ORC_ACC;
+                    if (I->max_step > 0) {
+                        double vmax2 = 0;
+                        for (int i = 0; i < n; ++i) {
+                            double v2 = v[3 * i] * v[3 * i] + v[3 * i + 1] * v[3 * i + 1] + v[3 * i + 2] * v[3 * i + 2];
+                            if (v2 > vmax2) vmax2 = v2;
+                        }
+                        if (dt * sqrt(vmax2) > I->max_step) {
+                            double sc2 = I->max_step / (dt * sqrt(vmax2));
+                            for (int i = 0; i < 3 * n; ++i) v[i] *= sc2;
+                        }
+                    }
+                    for (int i = 0; i < 3 * n; ++i) x[i] += dt * v[i];
+                    ++steps;
+                }
+                forces_free(g, T, I, x, F, E7);
+                double e = 0, fmax2 = 0;
+                for (int c = 0; c < 7; ++c) e += E7[c];
+                for (int i = 0; i < n; ++i) {
+                    double f2 = F[3 * i] * F[3 * i] + F[3 * i + 1] * F[3 * i + 1] + F[3 * i + 2] * F[3 * i + 2];
+                    if (f2 > fmax2) fmax2 = f2;
+                }
+                if (scan_out) {
+                    double* o = scan_out + ((long)r * I->n_scan + sc) * 4;
+                    o[0] = e; o[1] = it; o[2] = conv; o[3] = sqrt(fmax2);
+                }
+                flag += conv;
+            }
+        } else if (I->kind == 0) {
             /* velocity Verlet: v += dt/2 a; x += dt v; F(x); v += dt/2 a     (R13) */
-            orc_forces(g, T, x, F, E7);
+            forces_free(g, T, I, x, F, E7);
             if (e_trace) { double e = kinetic(T, v); for (int c = 0; c < 7; ++c) e += E7[c]; e_trace[(long)r * (I->n_steps + 1)] = e; }
             for (int s = 0; s < I->n_steps; ++s) {
                 for (int i = 0; i < n; ++i) for (int c = 0; c < 3; ++c) {
                     v[3 * i + c] += 0.5 * I->dt * F[3 * i + c] / T->mass[i] * ORC_ACC;
                     x[3 * i + c] += I->dt * v[3 * i + c];
                 }
-                orc_forces(g, T, x, F, E7);
+                forces_free(g, T, I, x, F, E7);
                 for (int i = 0; i < n; ++i) for (int c = 0; c < 3; ++c)
                     v[3 * i + c] += 0.5 * I->dt * F[3 * i + c] / T->mass[i] * ORC_ACC;
                 ++steps;
@@ -636,7 +749,7 @@ void orc_run_replicas(const orc_grid* g, const orc_topology* T, const orc_integr
             if (dt <= 0) { dt = I->dt; a = I->a_start; npos = 0; nrestart = 0; }
             int stopped = 0;
             for (int s = 0; s < I->n_steps; ++s) {
-                orc_forces(g, T, x, F, E7);
+                forces_free(g, T, I, x, F, E7);
                 double fmax2 = 0;
                 for (int i = 0; i < n; ++i) {
                     double f2 = F[3 * i] * F[3 * i] + F[3 * i + 1] * F[3 * i + 1] + F[3 * i + 2] * F[3 * i + 2];
@@ -688,7 +801,7 @@ void orc_run_replicas(const orc_grid* g, const orc_topology* T, const orc_integr
             }
             if (!stopped) {
                 /* energies (and, without restart, the converged flag) describe the final state */
-                orc_forces(g, T, x, F, E7);
+                forces_free(g, T, I, x, F, E7);
                 if (!I->restart) {
                     double fmax2 = 0;
                     for (int i = 0; i < n; ++i) {

@@ -50,7 +50,9 @@ class Integrator(C.Structure):
                 ("dt_max", C.c_double), ("f_inc", C.c_double), ("f_dec", C.c_double), ("a_start", C.c_double),
                 ("f_a", C.c_double), ("n_min", C.c_int), ("restart", C.c_int), ("seed", C.c_uint64),
                 ("z_ref", C.c_double), ("place_z_lo", C.c_double), ("place_z_hi", C.c_double),
-                ("place_z_min", C.c_double), ("clash", C.c_double), ("max_step", C.c_double)]
+                ("place_z_min", C.c_double), ("clash", C.c_double), ("max_step", C.c_double),
+                ("temperature", C.c_double), ("gamma", C.c_double), ("step0", C.c_uint32), ("n_scan", C.c_int),
+                ("fixed_mask", C.c_uint64), ("scan_dx", C.c_double * 3)]
 
 
 def lib():
@@ -209,12 +211,25 @@ class OracleTopology:
 
 
 def make_integrator(kind, n_steps, dt, f_tol=1e-3, dt_max=None, f_inc=1.1, f_dec=0.5, a_start=0.1, f_a=0.99,
-                    n_min=5, restart=0, seed=0, z_ref=0.0, place_z_lo=3.0, place_z_hi=6.0, place_z_min=2.0, clash=0.4, max_step=0.0):
-    kind = {"vv": 0, "fire": 1}.get(kind, kind)
+                    n_min=5, restart=0, seed=0, z_ref=0.0, place_z_lo=3.0, place_z_hi=6.0, place_z_min=2.0, clash=0.4, max_step=0.0,
+                    temperature=0.0, gamma=0.0, step0=0, n_scan=0, fixed=(), scan_dx=(0.0, 0.0, 0.0)):
+    """kind: "vv", "fire" or "langevin" (BAOAB, R18).  `fixed`: indices of held atoms; n_scan > 0 with kind "fire" = driven scan."""
+    kind = {"vv": 0, "fire": 1, "langevin": 2}.get(kind, kind)
+    mask = 0
+    for i in fixed:
+        mask |= 1 << int(i)
     if dt_max is None:
         dt_max = 10.0 * dt
     return Integrator(int(kind), int(n_steps), dt, f_tol, dt_max, f_inc, f_dec, a_start, f_a, int(n_min), int(restart),
-                      int(seed), z_ref, place_z_lo, place_z_hi, place_z_min, clash, max_step)
+                      int(seed), z_ref, place_z_lo, place_z_hi, place_z_min, clash, max_step,
+                      float(temperature), float(gamma), int(step0), int(n_scan), mask, (C.c_double * 3)(*[float(c) for c in scan_dx]))
+
+
+def langevin_normals(seed, replica, step, atom):
+    """the three standard normals the Langevin O-step draws for (replica, step, atom)"""
+    xi = np.zeros(3)
+    lib().orc_langevin_normals(C.c_uint64(int(seed)), C.c_uint32(int(replica)), C.c_uint32(int(step)), C.c_uint32(int(atom)), _p(xi))
+    return xi
 
 
 def intramolecular(otopo, pos):
@@ -246,7 +261,7 @@ def restart_conformation(otopo, integ, Lx, Ly, replica, restart, with_attempt=Fa
 
 
 def run_replicas(grid, otopo, integ, pos, vel, fire=None, minima_cap=0, trace=False):
-    """Returns dict(pos, vel, fire, energy[n_rep][8], status[n_rep][2], minima, n_minima, e_trace)."""
+    """Returns dict(pos, vel, fire, energy[n_rep][8], status[n_rep][2], minima, n_minima, e_trace, scan[n_rep][n_scan][4])."""
     n = otopo.n
     pos = _d(pos).reshape(-1, n, 3).copy(); vel = _d(vel).reshape(-1, n, 3).copy()
     n_rep = len(pos)
@@ -254,9 +269,10 @@ def run_replicas(grid, otopo, integ, pos, vel, fire=None, minima_cap=0, trace=Fa
     energy = np.zeros((n_rep, 8)); status = np.zeros((n_rep, 2), np.int32)
     minima = np.zeros((max(minima_cap, 1), 4 + 3 * n)); n_minima = C.c_long(0)
     e_trace = np.zeros((n_rep, integ.n_steps + 1)) if trace else None
+    scan = np.zeros((n_rep, integ.n_scan, 4)) if integ.n_scan > 0 else None
     lib().orc_run_replicas(C.byref(grid.c) if grid is not None else None, C.byref(otopo.c), C.byref(integ), C.c_int(n_rep),
                            _p(pos), _p(vel), _p(fire), _p(energy), _p(status),
-                           _p(minima) if minima_cap > 0 else None, C.c_long(minima_cap), C.byref(n_minima), _p(e_trace))
+                           _p(minima) if minima_cap > 0 else None, C.c_long(minima_cap), C.byref(n_minima), _p(e_trace), _p(scan))
     nm = int(n_minima.value)
     return dict(pos=pos, vel=vel, fire=fire, energy=energy, status=status,
-                minima=minima[:min(nm, minima_cap)], n_minima=nm, e_trace=e_trace)
+                minima=minima[:min(nm, minima_cap)], n_minima=nm, e_trace=e_trace, scan=scan)

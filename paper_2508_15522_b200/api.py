@@ -53,7 +53,9 @@ class Integrator(C.Structure):
                 ("dt_max", C.c_float), ("f_inc", C.c_float), ("f_dec", C.c_float), ("a_start", C.c_float), ("f_a", C.c_float),
                 ("n_min", C.c_int), ("max_step", C.c_float), ("restart", C.c_int), ("seed", C.c_ulonglong),
                 ("z_ref", C.c_float), ("place_z_lo", C.c_float), ("place_z_hi", C.c_float), ("place_z_min", C.c_float),
-                ("clash", C.c_float), ("variant", C.c_int)]
+                ("clash", C.c_float), ("variant", C.c_int),
+                ("temperature", C.c_float), ("gamma", C.c_float), ("step0", C.c_uint), ("n_scan", C.c_int),
+                ("fixed_mask", C.c_ulonglong), ("scan_dx", C.c_float * 3)]
 
 
 _vp, _sz, _ll, _i = C.c_void_p, C.c_size_t, C.c_longlong, C.c_int
@@ -77,6 +79,7 @@ _SIG = {
     "gridff_create_molecule": (_i, [_P(Topology), _vp, _sz, _vp, _P(_vp)]),
     "gridff_free_molecule": (_i, [_vp]),
     "gridff_run_replicas": (_i, [_vp, _vp, _P(Integrator), _i, _vp, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp]),
+    "gridff_run_scan": (_i, [_vp, _vp, _P(Integrator), _i, _vp, _vp, _vp, _vp, _vp, _vp]),
     "gridff_run_work_bytes": (_sz, [_vp, _i]),
     "gridff_run_replicas_host": (_i, [_vp, _vp, _P(Integrator), _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "gridff_probe_read": (_i, [_vp, _sz, _i, _i, _vp, _vp]),
@@ -322,12 +325,18 @@ def gridff_free_molecule(mol):
 
 
 def make_integrator(kind, n_steps, dt, f_tol=1e-3, dt_max=0.0, f_inc=1.1, f_dec=0.5, a_start=0.1, f_a=0.99, n_min=5,
-                    max_step=0.0, restart=0, seed=0, z_ref=0.0, place_z_lo=3.0, place_z_hi=6.0, place_z_min=2.0, clash=0.4, variant=0):
-    kind = {"vv": 0, "fire": 1}.get(kind, kind)
+                    max_step=0.0, restart=0, seed=0, z_ref=0.0, place_z_lo=3.0, place_z_hi=6.0, place_z_min=2.0, clash=0.4, variant=0,
+                    temperature=0.0, gamma=0.0, step0=0, n_scan=0, fixed=(), scan_dx=(0.0, 0.0, 0.0)):
+    """kind "vv" | "fire" | "langevin"; `fixed` = indices of held atoms; n_scan / scan_dx for gridff_run_scan."""
+    kind = {"vv": 0, "fire": 1, "langevin": 2}.get(kind, kind)
+    mask = 0
+    for i in fixed:
+        mask |= 1 << int(i)
     if not dt_max:
         dt_max = 10.0 * dt
     return Integrator(int(kind), int(n_steps), dt, f_tol, dt_max, f_inc, f_dec, a_start, f_a, int(n_min), max_step, int(restart),
-                      int(seed), z_ref, place_z_lo, place_z_hi, place_z_min, clash, int(variant))
+                      int(seed), z_ref, place_z_lo, place_z_hi, place_z_min, clash, int(variant),
+                      float(temperature), float(gamma), int(step0), int(n_scan), mask, (C.c_float * 3)(*[float(c) for c in scan_dx]))
 
 
 def gridff_run_replicas(grid, mol, integ, d_pos, d_vel, d_fire=None, d_energy=None, d_status=None, d_minima=None, d_n_minima=None,
@@ -342,6 +351,20 @@ def gridff_run_replicas(grid, mol, integ, d_pos, d_vel, d_fire=None, d_energy=No
     _check(_lib.gridff_run_replicas(None if grid is None else grid.handle, mol.handle, C.byref(integ), n_rep, _dptr(d_pos), _dptr(d_vel),
                                     _dptr(d_fire), _dptr(d_energy), _dptr(d_status), _dptr(d_minima), cap, _dptr(d_n_minima), _stream(stream)))
     return dict(energy=d_energy, status=d_status)
+
+
+def gridff_run_scan(grid, mol, integ, d_pos, d_vel, d_energy=None, d_status=None, d_scan=None, stream=None):
+    """driven scan (held atoms moved by integ.scan_dx, the rest relaxed, integ.n_scan times).  Returns dict(scan [n_rep][n_scan][4], energy, status)."""
+    n_rep = d_pos.shape[0]
+    if d_energy is None:
+        d_energy = torch.empty((n_rep, 8), dtype=torch.float32, device="cuda")
+    if d_status is None:
+        d_status = torch.empty((n_rep, 2), dtype=torch.int32, device="cuda")
+    if d_scan is None:
+        d_scan = torch.empty((n_rep, max(int(integ.n_scan), 0), 4), dtype=torch.float32, device="cuda")
+    _check(_lib.gridff_run_scan(None if grid is None else grid.handle, mol.handle, C.byref(integ), n_rep, _dptr(d_pos), _dptr(d_vel),
+                                _dptr(d_energy), _dptr(d_status), _dptr(d_scan), _stream(stream)))
+    return dict(scan=d_scan, energy=d_energy, status=d_status)
 
 
 def gridff_run_work_bytes(mol, n_rep):

@@ -394,28 +394,54 @@ def c4_points(n, Lx, Ly, z_lo_valid, z_hi_valid, seed=1004):
     return pos, coef
 
 
-def c4_samples(nx, ny, nz, h=0.1, z_lo=1.5, seed=1004, nch=3):
-    """smooth synthetic samples [nx][ny][nz][nch]: seeded sum of 8 plane-wave x exponential terms per channel.
-    (An input, like an imported density-derived grid; not a step of the method.)"""
+def c4_sample_terms(seed=1004, nch=3):
+    """parameters of the synthetic sweep potential: per channel 8 terms (m, n, phase, amplitude, decay)."""
     rng = np.random.default_rng(seed + 7)
-    x = (np.arange(nx) / nx)[:, None, None]; y = (np.arange(ny) / ny)[None, :, None]
-    z = (z_lo + h * np.arange(nz))[None, None, :]
-    out = np.zeros((nx, ny, nz, nch), np.float32)
+    terms = []
     for c in range(nch):
-        acc = np.zeros((nx, ny, nz))
+        ch = []
         for _ in range(8):
             m, n_ = rng.integers(0, 4, 2); ph = rng.uniform(0, 2 * math.pi); amp = rng.normal()
             kap = rng.uniform(0.3, 1.6)
-            acc += amp * np.cos(2 * math.pi * (m * x + n_ * y) + ph) * np.exp(-kap * (z - z_lo))
+            ch.append((int(m), int(n_), float(ph), float(amp), float(kap)))
+        terms.append(ch)
+    return terms
+
+
+def c4_samples(nx, ny, nz, h=0.1, z_lo=1.5, seed=1004, nch=3, xp=np, device=None):
+    """smooth synthetic samples [nx][ny][nz][nch]: seeded sum of 8 plane-wave x exponential terms per channel.
+    (An input, like an imported density-derived grid; not a step of the method.)  `xp` = numpy (default) or torch
+    (with `device`), so that the 512 x 512 x 256 sweep grid can be filled where it will live; same terms, same formula."""
+    terms = c4_sample_terms(seed, nch)
+    if xp is np:
+        ar = lambda n: np.arange(n, dtype=np.float64)
+        out = np.zeros((nx, ny, nz, nch), np.float32)
+    else:
+        ar = lambda n: xp.arange(n, dtype=xp.float64, device=device)
+        out = xp.zeros((nx, ny, nz, nch), dtype=xp.float32, device=device)
+    x = (ar(nx) / nx)[:, None, None]; y = (ar(ny) / ny)[None, :, None]
+    z = (z_lo + h * ar(nz))[None, None, :]
+    for c in range(nch):
+        acc = None
+        for (m, n_, ph, amp, kap) in terms[c]:
+            t = amp * xp.cos(2 * math.pi * (m * x + n_ * y) + ph) * xp.exp(-kap * (z - z_lo))
+            acc = t if acc is None else acc + t
         out[..., c] = acc
     return out
 
 
-def morton_order(pos, Lx, Ly, z0, nx, ny, hz):
-    """argsort of points by the Morton code of their grid cell (spatially sorted order for config 4)."""
-    ix = np.clip((pos[:, 0] / Lx * nx).astype(np.int64), 0, nx - 1)
-    iy = np.clip((pos[:, 1] / Ly * ny).astype(np.int64), 0, ny - 1)
-    iz = np.clip(((pos[:, 2] - z0) / hz).astype(np.int64), 0, (1 << 10) - 1)
+def morton_order(pos, Lx, Ly, z0, nx, ny, hz, xp=np):
+    """argsort of points by the Morton code of their grid cell (spatially sorted order for config 4).  `xp` = numpy, or torch for
+    points that already live on the device (2^26 of them sort in milliseconds there)."""
+    if xp is np:
+        i64 = lambda v: v.astype(np.int64)
+        clip = np.clip
+    else:
+        i64 = lambda v: v.to(xp.int64)
+        clip = xp.clamp
+    ix = clip(i64(pos[:, 0] / Lx * nx), 0, nx - 1)
+    iy = clip(i64(pos[:, 1] / Ly * ny), 0, ny - 1)
+    iz = clip(i64((pos[:, 2] - z0) / hz), 0, (1 << 10) - 1)
 
     def spread(v):
         v = v & 0x3FF
@@ -425,4 +451,4 @@ def morton_order(pos, Lx, Ly, z0, nx, ny, hz):
         v = (v | (v << 2)) & 0x9249249
         return v
     code = spread(iz) | (spread(iy) << 1) | (spread(ix) << 2)
-    return np.argsort(code, kind="stable")
+    return np.argsort(code, kind="stable") if xp is np else xp.argsort(code, stable=True)
