@@ -196,6 +196,40 @@ int gridff_run_replicas(const gridff_grid* grid, const gridff_molecule* mol, con
 int gridff_run_scan(const gridff_grid* grid, const gridff_molecule* mol, const gridff_integrator* integ, int n_rep,
                     float* d_pos, float* d_vel, float* d_energy, int* d_status, float* d_scan, void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * Minima hopping with an on-device unique-structure filter
+ * --------------------------------------------------------------------------------------------------------- */
+typedef struct {
+    int n_cycles;                       /* hops per call */
+    int cycle0;                         /* index of this call's first cycle (noise stream position = (cycle0 + c) * md_steps; record tag) */
+    int md_steps; float md_dt;          /* perturbation: Langevin dynamics from rest (1000 steps ...) */
+    float temperature, gamma;           /* ... at 300 K; friction 1/fs */
+    int relax_steps; float relax_dt;    /* FIRE relaxation from rest: at most relax_steps iterations */
+    float f_tol, dt_max, max_step;      /* FIRE: converged when max_i |F_i| < f_tol; dt_max 0 = 10 relax_dt; max_step 0 = none */
+    float e_tol, rmsd_tol;              /* same structure: |dE| < e_tol (1e-3 eV) and RMSD < rmsd_tol (0.1 Å) after removing the
+                                           whole cell translation nearest to the mean displacement (R16) */
+    unsigned long long seed;
+    unsigned long long fixed_mask;
+} gridff_hopping;
+
+/* n_cycles times, without host round-trips: Langevin -> FIRE -> filter.  Every replica continues from its relaxed state.
+ * The filter is the sequential greedy one in replica order: a converged replica whose structure matches no library record
+ * (older, or appended earlier in the same cycle) is appended.
+ *   d_pos      [n_rep][n][3]      in/out
+ *   d_library  [cap][4+3n]        in/out records {replica, cycle, FIRE iterations, E_total, positions}
+ *   d_n_library 1 int (device)    in/out number of records stored (<= cap)
+ *   d_stats    [n_cycles][4] int  out (may be NULL): converged candidates, new records, dropped because the library was full, library size after
+ *   d_work     gridff_hopping_work_bytes(mol, n_rep) bytes, 256-byte aligned                                           */
+size_t gridff_hopping_work_bytes(const gridff_molecule* mol, int n_rep);
+int gridff_minima_hopping(const gridff_grid* grid, const gridff_molecule* mol, const gridff_hopping* hop, int n_rep,
+                          float* d_pos, float* d_library, int cap, int* d_n_library, int* d_stats,
+                          void* d_work, size_t work_bytes, void* cuda_stream);
+/* The filter alone (parity hook and building block): candidates = replicas with d_ok[r] != 0, energies d_E [n_rep], positions d_pos. */
+int gridff_unique_filter(const gridff_grid* grid, const gridff_molecule* mol, int n_rep, const float* d_pos, const float* d_E,
+                         const int* d_steps /*may be NULL*/, const int* d_ok, float e_tol, float rmsd_tol, int tag,
+                         float* d_library, int cap, int* d_n_library, int* d_stats4 /*may be NULL*/,
+                         int* d_flags /*[n_rep] scratch*/, void* cuda_stream);
+
 /* Same through HOST buffers (pinned or pageable): copies pos/vel(/fire) to d_work, runs, copies pos/vel/fire/energy/
  * status back, synchronises the stream.  d_work needs gridff_run_work_bytes(mol, n_rep) bytes. */
 size_t gridff_run_work_bytes(const gridff_molecule* mol, int n_rep);

@@ -276,3 +276,56 @@ def run_replicas(grid, otopo, integ, pos, vel, fire=None, minima_cap=0, trace=Fa
     nm = int(n_minima.value)
     return dict(pos=pos, vel=vel, fire=fire, energy=energy, status=status,
                 minima=minima[:min(nm, minima_cap)], n_minima=nm, e_trace=e_trace, scan=scan)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# minima hopping with the unique-structure filter
+# ---------------------------------------------------------------------------------------------------------------
+
+def same_structure(E_a, x_a, E_b, x_b, Lx, Ly, e_tol=1e-3, rmsd_tol=0.1):
+    """PAPER.md:L241 criterion as read in DESIGN.md R16: |dE| < e_tol and plain RMSD < rmsd_tol (0.1 Å) after removing the whole
+    cell translation nearest to the mean displacement; no rotation, no atom permutation (adsorption site and orientation count)."""
+    if not abs(E_a - E_b) < e_tol:
+        return False
+    d = np.asarray(x_a, np.float64) - np.asarray(x_b, np.float64)
+    m = d.mean(axis=0)
+    d = d - np.array([round(m[0] / Lx) * Lx, round(m[1] / Ly) * Ly, 0.0])
+    return bool(np.sqrt((d ** 2).sum(axis=1).mean()) < rmsd_tol)
+
+
+def unique_filter(library, cand_E, cand_x, cand_ok, Lx, Ly, e_tol=1e-3, rmsd_tol=0.1, cap=None, tag=0, steps=None):
+    """Sequential greedy filter, candidates in replica order: a converged candidate that matches no library entry (old or added
+    earlier in this call) is appended as {replica, tag, steps, E, positions}.  `library` is a list of 1-D records [4 + 3n]; returns
+    (n_candidates, n_new, n_dropped)."""
+    n_cand = n_new = n_drop = 0
+    for r in range(len(cand_E)):
+        if not cand_ok[r]:
+            continue
+        n_cand += 1
+        x = np.asarray(cand_x[r], np.float64)
+        if any(same_structure(cand_E[r], x, rec[3], rec[4:].reshape(-1, 3), Lx, Ly, e_tol, rmsd_tol) for rec in library):
+            continue
+        if cap is not None and len(library) >= cap:
+            n_drop += 1
+            continue
+        library.append(np.concatenate([[r, tag, 0 if steps is None else steps[r], cand_E[r]], x.reshape(-1)]))
+        n_new += 1
+    return n_cand, n_new, n_drop
+
+
+def minima_hopping(grid, otopo, pos, n_cycles, md_steps, md_dt, temperature, gamma, relax_steps, relax_dt, f_tol, seed,
+                   dt_max=None, max_step=0.0, e_tol=1e-3, rmsd_tol=0.1, cap=None, cycle0=0, library=None):
+    """per cycle, `md_steps` of Langevin dynamics at `temperature` from the current state (noise stream step index
+    continues across cycles), FIRE relaxation from rest to max |F_i| < f_tol (at most relax_steps iterations), then the unique
+    filter; every replica continues from its relaxed state (R19).  Returns dict(pos, library, stats [n_cycles][3])."""
+    library = [] if library is None else library
+    pos = _d(pos).copy(); stats = []
+    for c in range(n_cycles):
+        md = make_integrator("langevin", md_steps, md_dt, temperature=temperature, gamma=gamma, seed=seed, step0=(cycle0 + c) * md_steps)
+        o = run_replicas(grid, otopo, md, pos, np.zeros_like(pos))
+        fi = make_integrator("fire", relax_steps, relax_dt, f_tol=f_tol, dt_max=dt_max, max_step=max_step)
+        o = run_replicas(grid, otopo, fi, o["pos"], np.zeros_like(pos))
+        pos = o["pos"]
+        E = o["energy"][:, :7].sum(axis=1)
+        stats.append(unique_filter(library, E, pos, o["status"][:, 1] == 1, grid.c.Lx, grid.c.Ly, e_tol, rmsd_tol, cap, cycle0 + c, o["status"][:, 0]))
+    return dict(pos=pos, library=library, stats=np.array(stats))
