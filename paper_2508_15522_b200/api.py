@@ -58,6 +58,13 @@ class Integrator(C.Structure):
                 ("fixed_mask", C.c_ulonglong), ("scan_dx", C.c_float * 3)]
 
 
+class Hopping(C.Structure):
+    _fields_ = [("n_cycles", C.c_int), ("cycle0", C.c_int), ("md_steps", C.c_int), ("md_dt", C.c_float),
+                ("temperature", C.c_float), ("gamma", C.c_float), ("relax_steps", C.c_int), ("relax_dt", C.c_float),
+                ("f_tol", C.c_float), ("dt_max", C.c_float), ("max_step", C.c_float), ("e_tol", C.c_float), ("rmsd_tol", C.c_float),
+                ("seed", C.c_ulonglong), ("fixed_mask", C.c_ulonglong)]
+
+
 _vp, _sz, _ll, _i = C.c_void_p, C.c_size_t, C.c_longlong, C.c_int
 _P = C.POINTER
 _SIG = {
@@ -80,6 +87,9 @@ _SIG = {
     "gridff_free_molecule": (_i, [_vp]),
     "gridff_run_replicas": (_i, [_vp, _vp, _P(Integrator), _i, _vp, _vp, _vp, _vp, _vp, _vp, _i, _vp, _vp]),
     "gridff_run_scan": (_i, [_vp, _vp, _P(Integrator), _i, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "gridff_hopping_work_bytes": (_sz, [_vp, _i]),
+    "gridff_minima_hopping": (_i, [_vp, _vp, _P(Hopping), _i, _vp, _vp, _i, _vp, _vp, _vp, _sz, _vp]),
+    "gridff_unique_filter": (_i, [_vp, _vp, _i, _vp, _vp, _vp, _vp, C.c_float, C.c_float, _i, _vp, _i, _vp, _vp, _vp, _vp]),
     "gridff_run_work_bytes": (_sz, [_vp, _i]),
     "gridff_run_replicas_host": (_i, [_vp, _vp, _P(Integrator), _i, _vp, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "gridff_probe_read": (_i, [_vp, _sz, _i, _i, _vp, _vp]),
@@ -365,6 +375,42 @@ def gridff_run_scan(grid, mol, integ, d_pos, d_vel, d_energy=None, d_status=None
     _check(_lib.gridff_run_scan(None if grid is None else grid.handle, mol.handle, C.byref(integ), n_rep, _dptr(d_pos), _dptr(d_vel),
                                 _dptr(d_energy), _dptr(d_status), _dptr(d_scan), _stream(stream)))
     return dict(scan=d_scan, energy=d_energy, status=d_status)
+
+
+def make_hopping(n_cycles, md_steps, md_dt, temperature, gamma, relax_steps, relax_dt, f_tol, seed, dt_max=0.0, max_step=0.0,
+                 e_tol=1e-3, rmsd_tol=0.1, cycle0=0, fixed=()):
+    mask = 0
+    for i in fixed:
+        mask |= 1 << int(i)
+    return Hopping(int(n_cycles), int(cycle0), int(md_steps), md_dt, temperature, gamma, int(relax_steps), relax_dt, f_tol, dt_max, max_step,
+                   e_tol, rmsd_tol, int(seed), mask)
+
+
+def gridff_hopping_work_bytes(mol, n_rep):
+    return int(_lib.gridff_hopping_work_bytes(mol.handle, int(n_rep)))
+
+
+def gridff_minima_hopping(grid, mol, hop, d_pos, d_library, d_n_library, d_stats=None, d_work=None, stream=None):
+    """hop.n_cycles x {Langevin, FIRE, unique filter} enqueued on the stream.  d_library [cap][4+3n] float32, d_n_library int32[1]
+    (both in/out), d_stats int32 [n_cycles][4].  Returns d_stats."""
+    n_rep = d_pos.shape[0]
+    if d_work is None:
+        d_work = _alloc(gridff_hopping_work_bytes(mol, n_rep))
+    if d_stats is None:
+        d_stats = torch.zeros((hop.n_cycles, 4), dtype=torch.int32, device="cuda")
+    _check(_lib.gridff_minima_hopping(grid.handle, mol.handle, C.byref(hop), n_rep, _dptr(d_pos), _dptr(d_library), d_library.shape[0],
+                                      _dptr(d_n_library), _dptr(d_stats), _dptr(d_work), d_work.numel(), _stream(stream)))
+    return d_stats
+
+
+def gridff_unique_filter(grid, mol, d_pos, d_E, d_ok, d_library, d_n_library, d_steps=None, e_tol=1e-3, rmsd_tol=0.1, tag=0, stream=None):
+    """the filter alone; returns int32[4] = candidates, new records, dropped (library full), library size after."""
+    n_rep = d_pos.shape[0]
+    stats = torch.zeros(4, dtype=torch.int32, device="cuda")
+    flags = torch.empty(n_rep, dtype=torch.int32, device="cuda")
+    _check(_lib.gridff_unique_filter(grid.handle, mol.handle, n_rep, _dptr(d_pos), _dptr(d_E), _dptr(d_steps), _dptr(d_ok), e_tol, rmsd_tol, int(tag),
+                                     _dptr(d_library), d_library.shape[0], _dptr(d_n_library), _dptr(stats), _dptr(flags), _stream(stream)))
+    return stats
 
 
 def gridff_run_work_bytes(mol, n_rep):

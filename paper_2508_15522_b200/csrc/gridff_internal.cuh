@@ -29,6 +29,7 @@ struct GridGeom {
 };
 
 struct MolDev;   // packed molecule in device memory (gridff_replica.cu)
+int molecule_n_atoms(const gridff_molecule* mol);     // gridff_replica.cu (the handle's layout is private to that file)
 
 void set_error(const char* fmt, ...);
 int cuda_fail(cudaError_t e, const char* what);
