@@ -46,6 +46,8 @@ def parse():
     ap.add_argument("--log2-points", type=int, default=26, help="config 4: number of interpolation points = 2^k")
     ap.add_argument("--order", default="random", choices=["random", "sorted"], help="config 4: point order (sorted = Morton order of the cell)")
     ap.add_argument("--c4-grid", default="config1", help="config 4: 'config1' (the 113 x 113 x 100 NaCl grid) or NXxNYxNZ synthetic sweep grid")
+    ap.add_argument("--c4-store", default="fp32", choices=["fp32", "half", "trilinear"],
+                    help="config 4: coefficient store read by gridff_eval: the fp32 spline (default), fp16 coefficients, or the paper's trilinear foil (SURVEY §8(f)3)")
     ap.add_argument("--sweep", action="store_true", help="config 4: also time the grid-size x order sweep (32^3 ... 512x512x256)")
     return ap.parse_args()
 
@@ -406,7 +408,16 @@ def run_eval(args):
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0)); hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6.65 TB/s (B200_PROFILING.md)"
 
-    def make_grid(desc, dims, sub):
+    def make_grid(desc, dims, sub, store="fp32"):
+        g0 = make_grid_fp32(desc, dims, sub)
+        if store == "fp32":
+            return g0
+        gd_ = api.gridff_grid_derive(g0, api.LAYOUT_HALF if store == "half" else api.LAYOUT_TRILINEAR)
+        torch.cuda.synchronize()
+        g0.free()
+        return gd_
+
+    def make_grid_fp32(desc, dims, sub):
         gd = api.make_desc(desc["Lx"], desc["Ly"], desc["z_ref"], desc["z_lo"], desc["z_hi"], desc["spacing"], desc["alpha"], desc["channels"],
                            r_cut=desc["r_cut"], l2_persist=1)
         if sub is not None:
@@ -446,8 +457,9 @@ def run_eval(args):
 
     name, dims, desc, sub = c4_grid_spec(args)
     n = 1 << args.log2_points
-    g = make_grid(desc, dims, sub)
+    g = make_grid(desc, dims, sub, args.c4_store)
     sb = g.store.numel()
+    bpe = BYTES_PER_EVAL if args.c4_store == "fp32" else 512          # half: 64 nodes x 8 B; trilinear foil: 8 nodes x 64 B
     pos, coef = make_points(desc, dims, n, shard.rank_seed(1004, rank))
     d_pos, d_coef = torch.from_numpy(pos).cuda(), torch.from_numpy(coef).cuda()
     z0 = desc["z_ref"] + desc["z_lo"]
@@ -497,9 +509,9 @@ def run_eval(args):
             dist.destroy_process_group()
         return
 
-    def roof(store_bytes, n_pts, ms, l2):
+    def roof(store_bytes, n_pts, ms, l2, bytes_per_eval=None):
         fits = store_bytes < (100 << 20)
-        ach = n_pts * float(BYTES_PER_EVAL) / (ms * 1e-3) / 1e9
+        ach = n_pts * float(bytes_per_eval or bpe) / (ms * 1e-3) / 1e9
         peak = l2["stream"] if fits else hbm_peak
         return fits, ach, peak
 
@@ -512,8 +524,9 @@ def run_eval(args):
     except Exception:
         pass
     roofline = {"bound": "l2" if fits else "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
-                "kernel": "k_eval_coop (warp-cooperative tricubic gather)", "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
-                "bytes_per_eval": BYTES_PER_EVAL, "evals_per_launch": n, "io_bytes_per_eval_hbm": C4_IO_BYTES,
+                "kernel": {"fp32": "k_eval_coop (warp-cooperative tricubic gather)", "half": "k_eval_half (tricubic, fp16 coefficients)",
+                           "trilinear": "k_eval_trilinear (8-corner foil, E and F tables)"}[args.c4_store], "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
+                "bytes_per_eval": bpe, "evals_per_launch": n, "io_bytes_per_eval_hbm": C4_IO_BYTES,
                 "io_stream_gbs": n * float(C4_IO_BYTES) / (kern_ms * 1e-3) / 1e9,
                 "peak_source": "L2 read bandwidth measured in this run by gridff_probe_read" if fits else hbm_src,
                 "l2_probe_gbs": l2, "hbm_peak_gbs": hbm_peak, "frac_of_hbm_peak": ach / hbm_peak}
@@ -524,24 +537,25 @@ def run_eval(args):
         del d_pos, d_coef
         specs = [("config1", dims, desc, sub)] + [("%dx%dx%d" % s_, s_, c4_synth_desc(*s_), None) for s_ in C4_SWEEP]
         for gname, gdims, gdesc, gsub in specs:
-            gg = make_grid(gdesc, gdims, gsub)
-            gsb = gg.store.numel()
-            gl2 = l2_probe(gsb) if gsb < (100 << 20) else l2
             p_, c_ = make_points(gdesc, gdims, n, 1004)
-            dp, dc = torch.from_numpy(p_).cuda(), torch.from_numpy(c_).cuda()
-            for order in ("random", "sorted"):
-                if order == "sorted":
-                    perm = inputs.morton_order(dp, gdesc["Lx"], gdesc["Ly"], gdesc["z_ref"] + gdesc["z_lo"], gdims[0], gdims[1], gdesc["spacing"], xp=torch)
-                    dp, dc = dp[perm].contiguous(), dc[perm].contiguous()
-                    del perm
-                t = float(np.mean(time_eval(gg, dp, dc, d_E, d_F, 3, 2)))
-                f_, a_, pk = roof(gsb, n, t, gl2)
-                sweep.append({"grid": gname, "store_MB": round(gsb / 1e6, 1), "order": order, "ms": t, "evals_per_s": n / (t * 1e-3),
-                              "gather_GBs": a_, "bound": "l2" if f_ else "hbm", "peak_GBs": pk, "frac": a_ / pk})
-                sys.stderr.write("sweep %-12s %7.1f MB %-6s %8.3f ms  %.3e evals/s  %8.1f GB/s  %.3f of %s\n"
-                                 % (gname, gsb / 1e6, order, t, n / (t * 1e-3), a_, a_ / pk, "l2" if f_ else "hbm"))
-            del dp, dc
-            gg.free()
+            dp0, dc0 = torch.from_numpy(p_).cuda(), torch.from_numpy(c_).cuda()
+            perm = inputs.morton_order(dp0, gdesc["Lx"], gdesc["Ly"], gdesc["z_ref"] + gdesc["z_lo"], gdims[0], gdims[1], gdesc["spacing"], xp=torch)
+            dp1, dc1 = dp0[perm].contiguous(), dc0[perm].contiguous()
+            del perm, p_, c_
+            for store in ("fp32", "half", "trilinear"):
+                gg = make_grid(gdesc, gdims, gsub, store)
+                gsb = gg.store.numel()
+                gl2 = l2_probe(gsb) if gsb < (100 << 20) else l2
+                sbpe = BYTES_PER_EVAL if store == "fp32" else 512
+                for order, dp, dc in (("random", dp0, dc0), ("sorted", dp1, dc1)):
+                    t = float(np.mean(time_eval(gg, dp, dc, d_E, d_F, 3, 2)))
+                    f_, a_, pk = roof(gsb, n, t, gl2, sbpe)
+                    sweep.append({"grid": gname, "store": store, "store_MB": round(gsb / 1e6, 1), "order": order, "ms": t, "evals_per_s": n / (t * 1e-3),
+                                  "bytes_per_eval": sbpe, "gather_GBs": a_, "bound": "l2" if f_ else "hbm", "peak_GBs": pk, "frac": a_ / pk})
+                    sys.stderr.write("sweep %-12s %-9s %7.1f MB %-6s %8.3f ms  %.3e evals/s  %8.1f GB/s  %.3f of %s\n"
+                                     % (gname, store, gsb / 1e6, order, t, n / (t * 1e-3), a_, a_ / pk, "l2" if f_ else "hbm"))
+                gg.free(); del gg
+            del dp0, dc0, dp1, dc1
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -562,7 +576,7 @@ def run_eval(args):
         "metric": C4_METRIC, "value": value, "unit": C4_UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "config4: 2^%d uniformly random points, %s, 3-channel E + analytic gradient" % (args.log2_points, name),
-                   "grid": list(dims), "store_bytes": sb, "points_per_gpu": n, "order": args.order, "parallelism": "points only (no collective)",
+                   "grid": list(dims), "store": args.c4_store, "store_bytes": sb, "points_per_gpu": n, "order": args.order, "parallelism": "points only (no collective)",
                    "l2_flush_between_steps": True, "step": "gridff_eval over all points (grid built before the timed region)"},
         "clocks": clocks, "e2e": {"value": e2e_value, "unit": C4_UNIT, "h2d_bytes_per_step": n * 28, "d2h_bytes_per_step": n * 16},
         "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "sweep": sweep}))

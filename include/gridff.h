@@ -48,7 +48,11 @@ typedef enum { GRIDFF_CH_PAULI = 0, GRIDFF_CH_LONDON = 1, GRIDFF_CH_COULOMB = 2,
 
 typedef enum {
     GRIDFF_LAYOUT_ZFAST = 0,  /* [x][y][z] nodes, z contiguous (the paper's order), x/y halo of 3 nodes */
-    GRIDFF_LAYOUT_BRICK = 1   /* 4x4x4-node bricks of 1 KB, bricks in [x][y][z] order, x/y halo                     */
+    GRIDFF_LAYOUT_BRICK = 1,  /* 4x4x4-node bricks of 1 KB, bricks in [x][y][z] order, x/y halo                     */
+    /* derived stores (gridff_grid_derive; gridff_eval only — SURVEY.md §8(f) row 3): */
+    GRIDFF_LAYOUT_HALF = 2,   /* ZFAST with the 4 coefficients of a node rounded to fp16 (8 B per node), fp32 arithmetic */
+    GRIDFF_LAYOUT_TRILINEAR = 3 /* the trilinear foil of PAPER.md:L118-120, L140: per node V and the three gradient components for
+                                   each channel (4 x float4 = 64 B), each interpolated independently over the 8 cell corners   */
 } gridff_layout;
 
 typedef struct {
@@ -95,6 +99,15 @@ int gridff_grid_info(const gridff_grid* grid, int dims[3], double h[3], double o
 
 /* Frees the handle only; d_store stays the caller's. */
 int gridff_free_grid(gridff_grid* grid);
+
+/* Derived stores for the interpolation trade study.  `parent` must be a ZFAST grid.
+ *   GRIDFF_LAYOUT_HALF       every stored fp32 coefficient rounded to nearest-even fp16; same tricubic evaluation, fp32 accumulate.
+ *   GRIDFF_LAYOUT_TRILINEAR  node values V_c = the parent spline at the node and G_c = its analytic gradient there (R20);
+ *                            gridff_eval then returns E = sum_c coef_c lerp(V_c), F = -sum_c coef_c lerp(G_c) ("the force components
+ *                            and energy were stored and interpolated independently", L120), cell and domain rules as for the spline.
+ * d_store (>= gridff_derive_bytes) stays the caller's; the handle is freed with gridff_free_grid.                          */
+size_t gridff_derive_bytes(const gridff_grid* parent, int layout);
+int gridff_grid_derive(const gridff_grid* parent, int layout, void* d_store, size_t store_bytes, void* cuda_stream, gridff_grid** out);
 
 /* Per-atom channel factors of PAPER.md:L83-85 Eq. 4 with e_i = sqrt(eps_i):
  *   coef[i] = { e_i exp(2 alpha R_i), -2 e_i exp(alpha R_i), q_i, 0 }.   HOST arrays, computed on the host in fp64. */

@@ -329,3 +329,63 @@ def minima_hopping(grid, otopo, pos, n_cycles, md_steps, md_dt, temperature, gam
         E = o["energy"][:, :7].sum(axis=1)
         stats.append(unique_filter(library, E, pos, o["status"][:, 1] == 1, grid.c.Lx, grid.c.Ly, e_tol, rmsd_tol, cap, cycle0 + c, o["status"][:, 0]))
     return dict(pos=pos, library=library, stats=np.array(stats))
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# interpolation variants — the trilinear foil and fp16 coefficient storage
+# ---------------------------------------------------------------------------------------------------------------
+
+def half_grid(grid):
+    """the same spline with every coefficient rounded fp64 -> fp32 -> fp16 (IEEE round-to-nearest-even, numpy's casts): what a
+    GRIDFF_LAYOUT_HALF store holds (it is derived from the fp32 store)."""
+    c = grid.coef.astype(np.float32).astype(np.float16).astype(np.float64)
+    return OracleGrid(c, grid.Lx, grid.Ly, grid.z0, grid.hz)
+
+
+def trilinear_nodes(grid):
+    """Node tables of the foil (R20): V [nx][ny][nz][C] = the spline at the nodes, G [nx][ny][nz][C][3] = its analytic
+    gradient there, for iz in [1, nz-2]; zero at iz = 0 and nz-1 (not needed: cells are clamped to [1, nz-3]).  At a node the
+    cubic B-spline weights are B(-1), B(0), B(1) = 1/6, 2/3, 1/6 and B'(1), B'(0), B'(-1) = -1/2, 0, 1/2 (Eq. 6)."""
+    nx, ny, nz, nch = grid.shape
+    b = grid.coef
+    w = (1.0 / 6.0, 2.0 / 3.0, 1.0 / 6.0); d = (-0.5, 0.0, 0.5)
+    h = (grid.Lx / nx, grid.Ly / ny, grid.hz)
+    V = np.zeros((nx, ny, nz, nch)); G = np.zeros((nx, ny, nz, nch, 3))
+    for a in range(3):
+        for bb in range(3):
+            for c in range(3):
+                # coefficient (i - 1 + a, j - 1 + bb, k - 1 + c): periodic in x, y; k = 1 .. nz-2 in z
+                blk = np.roll(np.roll(b, 1 - a, axis=0), 1 - bb, axis=1)[:, :, c:nz - 2 + c]
+                V[:, :, 1:nz - 1] += w[a] * w[bb] * w[c] * blk
+                G[:, :, 1:nz - 1, :, 0] += d[a] * w[bb] * w[c] / h[0] * blk
+                G[:, :, 1:nz - 1, :, 1] += w[a] * d[bb] * w[c] / h[1] * blk
+                G[:, :, 1:nz - 1, :, 2] += w[a] * w[bb] * d[c] / h[2] * blk
+    return V, G
+
+
+def interp_trilinear(grid, nodes, pos, coef):
+    """energy and the three force components stored on the grid and interpolated independently, trilinearly over the 8
+    corners of the cell.  Cell and domain rules are the spline's (R5, R6): x, y periodic, i_z clamped to [1, nz-3] with
+    t_z = u_z - i_z (linear continuation below), E = F = 0 for u_z >= nz - 2.  Returns (E [n], F [n][3])."""
+    V, G = nodes
+    nx, ny, nz, nch = grid.shape
+    pos = _d(pos).reshape(-1, 3); coef = _d(coef).reshape(len(pos), 4)
+    E = np.zeros(len(pos)); F = np.zeros((len(pos), 3))
+    for p in range(len(pos)):
+        ux = (pos[p, 0] / grid.Lx - np.floor(pos[p, 0] / grid.Lx)) * nx
+        uy = (pos[p, 1] / grid.Ly - np.floor(pos[p, 1] / grid.Ly)) * ny
+        uz = (pos[p, 2] - grid.z0) / grid.hz
+        if uz >= nz - 2:
+            continue
+        ix = min(int(np.floor(ux)), nx - 1); iy = min(int(np.floor(uy)), ny - 1)
+        iz = min(max(int(np.floor(uz)), 1), nz - 3)
+        tx, ty, tz = ux - ix, uy - iy, uz - iz
+        for a in (0, 1):
+            for b in (0, 1):
+                for c in (0, 1):
+                    w = (tx if a else 1 - tx) * (ty if b else 1 - ty) * (tz if c else 1 - tz)
+                    jx, jy, jz = (ix + a) % nx, (iy + b) % ny, iz + c
+                    for ch in range(nch):
+                        E[p] += coef[p, ch] * w * V[jx, jy, jz, ch]
+                        F[p] -= coef[p, ch] * w * G[jx, jy, jz, ch]
+    return E, F

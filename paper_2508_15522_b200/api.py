@@ -77,6 +77,8 @@ _SIG = {
     "gridff_grid_export": (_i, [_vp, _vp, _vp]),
     "gridff_grid_info": (_i, [_vp, _P(_i * 3), _P(C.c_double * 3), _P(C.c_double * 3), _P(_i), _P(_i)]),
     "gridff_free_grid": (_i, [_vp]),
+    "gridff_derive_bytes": (_sz, [_vp, _i]),
+    "gridff_grid_derive": (_i, [_vp, _i, _vp, _sz, _vp, _P(_vp)]),
     "gridff_atom_coefs": (_i, [C.c_double, _i, _vp, _vp, _vp, _vp]),
     "gridff_eval": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp]),
     "gridff_eval_variant": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _i, _vp]),
@@ -219,6 +221,18 @@ def gridff_grid_from_samples(desc, d_samples, stream=None):
                                          _stream(stream), C.byref(out)))
     torch.cuda.current_stream().synchronize()
     return Grid(out, desc, store)
+
+
+LAYOUT_HALF, LAYOUT_TRILINEAR = 2, 3
+
+
+def gridff_grid_derive(parent, layout, stream=None):
+    """derived store for the interpolation trade study: LAYOUT_HALF (fp16 coefficients) or LAYOUT_TRILINEAR (the paper's foil); gridff_eval only."""
+    nbytes = int(_lib.gridff_derive_bytes(parent.handle, int(layout)))
+    store = _alloc(nbytes)
+    out = C.c_void_p(None)
+    _check(_lib.gridff_grid_derive(parent.handle, int(layout), _dptr(store), store.numel(), _stream(stream), C.byref(out)))
+    return Grid(out, parent.desc, store)
 
 
 def gridff_grid_export(grid, stream=None):

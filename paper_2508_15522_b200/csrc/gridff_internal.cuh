@@ -6,6 +6,8 @@
 #include <stddef.h>
 #include "../../include/gridff.h"
 
+struct gridff_grid;
+
 namespace gridff {
 
 constexpr double kKe = 14.3996454784;      // eV·Å/e²
@@ -32,6 +34,7 @@ struct MolDev;   // packed molecule in device memory (gridff_replica.cu)
 int molecule_n_atoms(const gridff_molecule* mol);     // gridff_replica.cu (the handle's layout is private to that file)
 
 void set_error(const char* fmt, ...);
+int eval_derived(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);   // gridff_derive.cu
 int cuda_fail(cudaError_t e, const char* what);
 void count_launch(int n = 1);
 

@@ -304,16 +304,19 @@ def _twist(pos, topo, rng, clash=0.6, tries=256):
     return best
 
 
-def place_replicas(topo, n_rep, Lx, Ly, z_ref, seed, z_lo=3.0, z_hi=6.0, z_min=2.0, twist=False):
+def place_replicas(topo, n_rep, Lx, Ly, z_ref, seed, z_lo=3.0, z_hi=6.0, z_min=2.0, twist=False, twist_pool=256):
     """centroid x,y ~ U(0,L), orientation uniform on SO(3), centroid z ~ U(z_lo, z_hi) above z_ref, lifted so the
-    lowest atom is >= z_min above z_ref.  Returns float32 [n_rep][n][3]."""
+    lowest atom is >= z_min above z_ref.  Returns float32 [n_rep][n][3].  With `twist`, every replica gets its own clash-free random
+    dihedrals while n_rep <= twist_pool; larger batches draw twist_pool conformers and replica r takes conformer r mod twist_pool
+    (its orientation and placement stay its own) — the clash-free re-draws are a Python loop, ~80 ms each."""
     rng = np.random.default_rng(seed)
     n = topo["n_atoms"]
     ref = np.asarray(topo["ref_pos"], dtype=np.float64)
     rots = _random_rotations(rng, n_rep)
     out = np.zeros((n_rep, n, 3))
+    pool = [_twist(ref, topo, rng) for _ in range(twist_pool)] if (twist and n_rep > twist_pool) else None
     for r in range(n_rep):
-        p = _twist(ref, topo, rng) if twist else ref
+        p = pool[r % twist_pool] if pool is not None else (_twist(ref, topo, rng) if twist else ref)
         p = (p - p.mean(axis=0)) @ rots[r].T
         p = p + np.array([rng.uniform(0, Lx), rng.uniform(0, Ly), z_ref + rng.uniform(z_lo, z_hi)])
         lift = z_ref + z_min - p[:, 2].min()

@@ -1,0 +1,86 @@
+"""GPU-vs-oracle parity for the derived stores of the interpolation trade study: fp16 coefficients
+(GRIDFF_LAYOUT_HALF) and the trilinear foil of PAPER.md:L118-120 (GRIDFF_LAYOUT_TRILINEAR), through gridff_grid_derive + gridff_eval.
+Run on the B200 box with -m gpu.  Tolerances are north_star's for interpolation: energy 1e-5 relative (denominator sum_c |coef_c V_c|
+widened to the magnitude of the coefficients that enter, R14), force 1e-4 eV/Å — each variant against the oracle's
+statement of THAT variant (same rounded coefficients / same node tables), so the comparison isolates the fp32 arithmetic."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2508_15522_b200 import inputs
+from gridff_cases import oracle_grid, gpu_grid, small_config
+from test_gpu_parity import api, dev, cfg1s, eval_points  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+def test_half_store_parity(api, orc, cfg1s):
+    og, _ = oracle_grid(orc, cfg1s["sub"], cfg1s["desc"])
+    g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
+    gh = api.gridff_grid_derive(g, api.LAYOUT_HALF)
+    # the oracle rounds the GPU's own fp32 coefficients?  No: its own fp64 -> fp32 -> fp16.  The two fp32 stores agree to ~1e-7 relative,
+    # so a coefficient can land on the other side of an fp16 rounding boundary (1 in ~10^4): compare on the oracle's rounding of the
+    # exported GPU coefficients for the bit-level check, and on its own for the end-to-end one.
+    coef32 = api.gridff_grid_export(g).cpu().numpy()
+    hg_same = orc.OracleGrid(coef32.astype(np.float16).astype(np.float64), og.Lx, og.Ly, og.z0, og.hz)
+    pos, cf = eval_points(cfg1s, 20011, 5)                        # ragged tail, many blocks
+    E, F = api.gridff_eval(gh, dev(pos), dev(cf))
+    E, F = E.cpu().numpy(), F.cpu().numpy()
+    Eo, Fo, Vc, _ = orc.interp(hg_same, pos, cf, channels=True)
+    den = np.maximum(np.sum(np.abs(cf[:, :3].astype(np.float64) * Vc), axis=1), 1e-12)       # points above the domain: E = den = 0
+    assert (np.abs(E - Eo) / den).max() <= 1e-5
+    assert np.abs(F - Fo).max() <= 1e-4
+    # end to end against the oracle's own half grid: within the fp16 quantisation of a few boundary coefficients
+    Eh, Fh = orc.interp(orc.half_grid(og), pos, cf)
+    assert (np.abs(E - Eh) / den).max() <= 2e-3 and np.median(np.abs(E - Eh) / den) <= 1e-6
+    # and the price of fp16 against the full-precision spline (reported)
+    Ef, Ff = orc.interp(og, pos, cf)
+    print("fp16 store vs fp64 spline: median rel E err %.2e, max %.2e; max |dF| %.2e eV/A"
+          % (np.median(np.abs(E - Ef) / den), (np.abs(E - Ef) / den).max(), np.abs(F - Ff).max()))
+    with pytest.raises(api.GridffError):
+        api.gridff_grid_export(gh)
+
+
+def test_trilinear_foil_parity(api, orc, cfg1s):
+    og, _ = oracle_grid(orc, cfg1s["sub"], cfg1s["desc"])
+    g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
+    gt = api.gridff_grid_derive(g, api.LAYOUT_TRILINEAR)
+    nodes = orc.trilinear_nodes(og)
+    pos, cf = eval_points(cfg1s, 6007, 6)
+    # include edge cases: exactly on nodes, periodic images, below node 1 (linear continuation), above the domain (zero)
+    nz = og.shape[2]
+    pos[:50, 0] = np.round(pos[:50, 0] / (og.Lx / og.shape[0])) * np.float32(og.Lx / og.shape[0])
+    pos[50:100, 0] += np.float32(3 * og.Lx); pos[100:150, 1] -= np.float32(2 * og.Ly)
+    pos[150:170, 2] = np.float32(og.z0 + 0.6 * og.hz)
+    pos[170:190, 2] = np.float32(og.z0 + (nz - 2) * og.hz + 0.05)
+    E, F = api.gridff_eval(gt, dev(pos), dev(cf))
+    E, F = E.cpu().numpy(), F.cpu().numpy()
+    Eo, Fo = orc.interp_trilinear(og, nodes, pos.astype(np.float64), cf.astype(np.float64))
+    _, _, Vc, _ = orc.interp(og, pos, cf, channels=True)
+    den = np.maximum(np.sum(np.abs(cf[:, :3].astype(np.float64) * Vc), axis=1), 1e-6)
+    assert (np.abs(E - Eo) / den).max() <= 1e-5, (np.abs(E - Eo) / den).max()
+    assert np.abs(F - Fo).max() <= 1e-4
+    assert np.all(E[170:190] == 0) and np.all(F[170:190] == 0)
+    # the trade the paper describes (L140): orders of magnitude less accurate than the spline
+    Es, Fs = orc.interp(og, pos, cf)
+    sel = slice(190, None)
+    print("trilinear foil vs spline: max |dE| %.2e eV, max |dF| %.2e eV/A (spline fp32 path: 1e-6 / 1e-5)"
+          % (np.abs(E[sel] - Es[sel]).max(), np.abs(F[sel] - Fs[sel]).max()))
+    assert np.abs(E[sel] - Es[sel]).max() > 1e-4
+
+
+def test_derive_errors(api, cfg1s):
+    g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
+    gb = gpu_grid(api, cfg1s["sub"], cfg1s["desc"], layout=1)
+    with pytest.raises(api.GridffError):
+        api.gridff_grid_derive(gb, api.LAYOUT_HALF)               # brick parent
+    with pytest.raises(api.GridffError):
+        api.gridff_grid_derive(g, 7)
+    gh = api.gridff_grid_derive(g, api.LAYOUT_HALF)
+    with pytest.raises(api.GridffError):
+        api.gridff_grid_derive(gh, api.LAYOUT_TRILINEAR)          # derived from derived
+    # the replica kernel refuses derived stores
+    topo = cfg1s["topo"]
+    mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(cfg1s["desc"]["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
+    with pytest.raises(api.GridffError):
+        api.gridff_run_replicas(gh, mol, api.make_integrator("vv", 1, 0.5), dev(cfg1s["pos"]), dev(cfg1s["vel"]))
