@@ -43,6 +43,9 @@ def parse():
     ap.add_argument("--replicas", type=int, default=0, help="override the config's replica count (0 = config value)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="run", choices=["run", "langevin", "hopping", "scan"],
+                    help="SURVEY §8(f) rows on the chosen replica config: langevin = kind 2 instead of the config's integrator; hopping = "
+                         "gridff_minima_hopping cycles (1000 Langevin steps at 300 K + FIRE); scan = gridff_run_scan lift of one held atom")
     ap.add_argument("--log2-points", type=int, default=26, help="config 4: number of interpolation points = 2^k")
     ap.add_argument("--order", default="random", choices=["random", "sorted"], help="config 4: point order (sorted = Morton order of the cell)")
     ap.add_argument("--c4-grid", default="config1", help="config 4: 'config1' (the 113 x 113 x 100 NaCl grid) or NXxNYxNZ synthetic sweep grid")
@@ -143,6 +146,61 @@ class ClockSampler:
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx or None, "power_w_max": pw or None,
                 "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_f_rows(args):
+    """--mode langevin | hopping | scan: device-timed throughput of the §8(f) entry points on the config's grid and molecule (one GPU)."""
+    import torch
+    from paper_2508_15522_b200 import api
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(0)
+    cfg, md, dims, name = workload(args)
+    d, topo, sub = cfg["desc"], cfg["topo"], cfg["sub"]
+    n_rep, n_at = cfg["n_rep"], int(topo["n_atoms"])
+    g = api.gridff_build_grid(api.make_desc(d["Lx"], d["Ly"], d["z_ref"], d["z_lo"], d["z_hi"], d["spacing"], d["alpha"], d["channels"], r_cut=d["r_cut"], l2_persist=1),
+                              sub["pos"], sub["e"], sub["R"], sub["q"])
+    mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
+    pos0 = torch.from_numpy(cfg["pos"]).cuda()
+    stream = torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    l0 = api.gridff_launch_count()
+    extra = {}
+    ts = []
+    for it in range(max(args.warmup, 3) + args.steps):
+        d_pos = pos0.clone(); d_vel = torch.zeros_like(d_pos)
+        flush.fill_(1)
+        a, b = ev(), ev()
+        if args.mode == "langevin":
+            integ = api.make_integrator("langevin", md, 0.5, temperature=300.0, gamma=0.01, seed=7)
+            a.record(stream); api.gridff_run_replicas(g, mol, integ, d_pos, d_vel); b.record(stream); b.synchronize()
+            units = n_rep * md
+        elif args.mode == "hopping":
+            cycles = 2
+            hop = api.make_hopping(cycles, 1000, 0.5, 300.0, 0.01, 5000, 1.0, 1e-3, seed=7, dt_max=20.0, max_step=0.1)
+            d_lib = torch.zeros((4 * n_rep, 4 + 3 * n_at), device="cuda"); d_n = torch.zeros(1, dtype=torch.int32, device="cuda")
+            d_work = torch.empty(api.gridff_hopping_work_bytes(mol, n_rep), dtype=torch.uint8, device="cuda")
+            a.record(stream); st = api.gridff_minima_hopping(g, mol, hop, d_pos, d_lib, d_n, d_work=d_work); b.record(stream); b.synchronize()
+            st = st.cpu().numpy()
+            units = n_rep * cycles                       # hops
+            extra = {"cycles": cycles, "md_steps": 1000, "relax_cap": 5000, "stats_per_cycle[candidates,new,dropped,library]": st.tolist()}
+        else:
+            n_scan = 20
+            integ = api.make_integrator("fire", 2000, 1.0, f_tol=2e-3, dt_max=10.0, max_step=0.05, n_scan=n_scan, fixed=(n_at - 1,), scan_dx=(0.0, 0.0, 0.1))
+            a.record(stream); out = api.gridff_run_scan(g, mol, integ, d_pos, d_vel); b.record(stream); b.synchronize()
+            units = int(out["status"][:, 0].sum().item())        # FIRE iterations really taken
+            extra = {"n_scan": n_scan, "points_converged_frac": float(out["scan"][..., 2].mean().item()), "scan_points_per_s": None}
+        if it >= max(args.warmup, 3):
+            ts.append(a.elapsed_time(b))
+    ms = float(np.mean(ts))
+    if args.mode == "scan":
+        extra["scan_points_per_s"] = n_rep * extra["n_scan"] / (ms * 1e-3)
+    unit = {"langevin": "replica-steps/s", "hopping": "hops/s", "scan": "replica-steps/s"}[args.mode]
+    print(json.dumps({"metric": {"langevin": "replica_md_steps_per_s", "hopping": "minima_hops_per_s", "scan": "replica_md_steps_per_s"}[args.mode],
+                      "value": units / (ms * 1e-3), "unit": unit, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                      "config": {"workload": "%s [mode %s]" % (name, args.mode), "n_replicas_per_gpu": n_rep, "atoms": n_at, "l2_flush_between_steps": True},
+                      "gpu_launches": int(api.gridff_launch_count() - l0), "details": extra}))
 
 
 def run_gridff(args):
@@ -589,4 +647,7 @@ if __name__ == "__main__":
     if a.impl == "reference":
         run_eval_reference(a) if a.config == 4 else run_reference(a)
     else:
-        run_eval(a) if a.config == 4 else run_gridff(a)
+        if a.mode != "run" and a.config != 4:
+            run_f_rows(a)
+        else:
+            run_eval(a) if a.config == 4 else run_gridff(a)
