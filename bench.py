@@ -73,10 +73,21 @@ def oracle_sample(cfg, md_steps, n_rep_sample=64, steps_sample=200):
     steps_sample steps (a5-a9).  Returns (t_build, t_per_replica_step, cores)."""
     from oracle import gridff_oracle as orc
     d = cfg["desc"]; nx, ny, nz = inputs.grid_dims(d); z0 = d["z_ref"] + d["z_lo"]
+    # bounded sample of the build: the direct sums cost nodes x atoms x images; above ~2e10 pair terms (config 3: 2.6e11) only the lowest
+    # nz_s z-planes are built and the sampling time is scaled by nz / nz_s (it is linear in the node count)
+    n_img = int(np.prod([2 * int(np.ceil(d["r_cut"] / L)) + 1 for L in (d["Lx"], d["Ly"])]))
+    work = float(nx) * ny * nz * len(cfg["sub"]["pos"]) * n_img
+    nz_s = nz if work <= 2e10 else max(8, int(nz * 2e10 / work))
     t0 = time.perf_counter()
-    samples = orc.sample_grid(cfg["sub"], d["alpha"], d["Lx"], d["Ly"], d["r_cut"], nx, ny, nz, z0, d["spacing"], d["channels"])
+    samples = orc.sample_grid(cfg["sub"], d["alpha"], d["Lx"], d["Ly"], d["r_cut"], nx, ny, nz_s, z0, d["spacing"], d["channels"])
+    t_sample = time.perf_counter() - t0
+    if nz_s < nz:
+        # the run leg needs a grid under the molecules: prefilter (timed, full size) smooth synthetic samples of the config's dimensions —
+        # interpolation cost does not depend on the values
+        samples = inputs.c4_samples(nx, ny, nz, h=d["spacing"], z_lo=d["z_lo"], nch=len(d["channels"])).astype(np.float64)
+    t0 = time.perf_counter()
     og = orc.OracleGrid(orc.prefilter(samples, (1, 1, 0)), d["Lx"], d["Ly"], z0, d["spacing"])
-    t_build = time.perf_counter() - t0
+    t_build = t_sample * nz / nz_s + (time.perf_counter() - t0)
     topo = cfg["topo"]
     ot = orc.OracleTopology(topo, orc.atom_coefs(topo["grid_e"], topo["grid_R"], topo["q"], d["alpha"]))
     kind = cfg["integ"]["kind"]

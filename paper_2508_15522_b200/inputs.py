@@ -272,6 +272,20 @@ def chain60(seed=1002):
 
 # ----------------------------------------------------------------------------- placements
 
+def helix_chain(n, seed=7):
+    """n-atom united-atom chain (C, C, O repeating) wound as a loose helix (bond 1.5 Å, angle 112 deg, dihedral 70 deg): bonds i-(i+1),
+    all angles, one n = 3 torsion per 4 consecutive atoms, partial charges, LJ + Coulomb beyond 3 bonds.  A size-parametrised molecule
+    for the edge cases of the replica kernel (1, 2, 3, 32, 33, 64 atoms); not one of the BASELINE configs."""
+    rng = np.random.default_rng(seed)
+    el = [("C", "C", "O")[i % 3] for i in range(n)]
+    pos = [np.zeros(3), np.array([1.5, 0.0, 0.0]), np.array([1.5 + 1.5 * math.cos(math.radians(68)), 1.5 * math.sin(math.radians(68)), 0.0])][:n]
+    for i in range(3, n):
+        pos.append(_nerf(pos[i - 3], pos[i - 2], pos[i - 1], 1.5, math.radians(112), math.radians(70)))
+    bonds = [(i, i + 1) for i in range(n - 1)]
+    tors = [(i, i + 1, i + 2, i + 3, 0.03, 3.0, 0.0) for i in range(n - 3)]
+    return _finish(el, np.array(pos), bonds, _bond_k, tors, [], rng, True, True)
+
+
 def _random_rotations(rng, n):
     q = rng.normal(size=(n, 4)); q /= np.linalg.norm(q, axis=1, keepdims=True)
     x, y, z, w = q.T

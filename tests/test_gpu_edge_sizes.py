@@ -1,0 +1,56 @@
+"""Edge sizes of the fused replica kernel (run on the B200 box with -m gpu): molecules of 1, 2, 3, 4, 32 (a full warp, one atom per
+lane), 33 (the first size with two atoms per lane), 61 and 64 (the maximum) atoms; replica counts of 1 and one more than a whole number
+of blocks; zero replicas and zero steps.  Energies at the fixed state and 40-step velocity-Verlet and Langevin trajectories against
+the oracle, on the small config-1 grid."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2508_15522_b200 import inputs
+from gridff_cases import oracle_grid, gpu_grid, small_config
+from test_gpu_parity import api, dev, run_gpu, check_energies, TRAJ_TOL  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("n_atoms,n_rep", [(1, 5), (2, 8), (3, 15), (4, 1), (32, 29), (33, 17), (61, 9), (64, 10)])
+def test_molecule_sizes(api, orc, n_atoms, n_rep):
+    cfg = small_config(1, n_rep=1)
+    d = cfg["desc"]
+    og, _ = oracle_grid(orc, cfg["sub"], d)
+    g = gpu_grid(api, cfg["sub"], d)
+    topo = inputs.helix_chain(n_atoms, seed=100 + n_atoms)
+    ot = orc.OracleTopology(topo, orc.atom_coefs(topo["grid_e"], topo["grid_R"], topo["q"], d["alpha"]))
+    mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
+    pos = inputs.place_replicas(topo, n_rep, d["Lx"], d["Ly"], 0.0, 77 + n_atoms)
+    vel = inputs.maxwell_boltzmann(topo, n_rep, 300.0, 78)
+    r0 = run_gpu(api, g, mol, api.make_integrator("vv", 0, 0.5), pos, vel)
+    o0 = orc.run_replicas(og, ot, orc.make_integrator("vv", 0, 0.5), pos, vel)
+    check_energies(r0["energy"], o0["energy"], tol_rel=3e-5, tol_abs=3e-5)
+    for kind, kw in (("vv", {}), ("langevin", dict(temperature=300.0, gamma=0.02, seed=5))):
+        r = run_gpu(api, g, mol, api.make_integrator(kind, 40, 0.5, **kw), pos, vel)
+        o = orc.run_replicas(og, ot, orc.make_integrator(kind, 40, 0.5, **kw), pos, vel)
+        assert np.abs(r["pos"].astype(np.float64) - o["pos"]).max() <= TRAJ_TOL, (kind, n_atoms)
+        check_energies(r["energy"], o["energy"], tol_rel=1e-4, tol_abs=2e-4)
+    # every variant agrees on the forces: 40 steps bit-identical between the cached and the gather-every-step kernels
+    r2 = run_gpu(api, g, mol, api.make_integrator("vv", 40, 0.5, variant=2), pos, vel)
+    r3 = run_gpu(api, g, mol, api.make_integrator("vv", 40, 0.5, variant=3), pos, vel)
+    assert np.array_equal(r2["pos"], r3["pos"])
+
+
+def test_zero_replicas_and_too_many_atoms(api):
+    cfg = small_config(1, n_rep=1)
+    d = cfg["desc"]
+    g = gpu_grid(api, cfg["sub"], d)
+    topo = inputs.helix_chain(5)
+    mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
+    empty = torch.zeros((0, 5, 3), device="cuda")
+    out = api.gridff_run_replicas(g, mol, api.make_integrator("vv", 10, 0.5), empty, empty.clone())
+    assert out["energy"].shape == (0, 8)
+    E, F = api.gridff_eval(g, torch.zeros((0, 3), device="cuda"), torch.zeros((0, 4), device="cuda"))
+    assert E.shape == (0,) and F.shape == (0, 3)
+    big65 = inputs.helix_chain(65)
+    with pytest.raises(api.GridffError):
+        api.gridff_create_molecule(big65, np.zeros((65, 4), np.float32))
+    with pytest.raises(api.GridffError):
+        api.gridff_run_replicas(g, mol, api.make_integrator("vv", 10, 0.5, fixed=(7,)), dev(np.zeros((2, 5, 3))), dev(np.zeros((2, 5, 3))))
