@@ -130,7 +130,9 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
                         float* d_E, float* d_F, int variant, void* cuda_stream);
 
 /* Same through HOST buffers: copies pos/coef to d_work, evaluates, copies E/F back, synchronises the stream.
- * d_work needs gridff_eval_work_bytes(n) bytes. */
+ * d_work needs gridff_eval_work_bytes(n) bytes.  The work is pipelined in chunks of 2^22 points over two library-owned copy streams
+ * and the caller's stream (upload of chunk c+1, kernel of chunk c and download of chunk c-1 overlap); the overlap needs pinned
+ * host buffers, pageable ones are correct but serialise. */
 size_t gridff_eval_work_bytes(long long n);
 int gridff_eval_host(const gridff_grid* grid, long long n, const float* h_pos, const float* h_coef,
                      float* h_E, float* h_F, void* d_work, size_t work_bytes, void* cuda_stream);

@@ -177,12 +177,41 @@ int gridff_eval_host(const gridff_grid* grid, long long n, const float* h_pos, c
     float* d_pos = (float*)(w + (size_t)n * 16);     // [n][3]
     float* d_F = (float*)(w + (size_t)n * 28);       // [n][3]
     float* d_E = (float*)(w + (size_t)n * 40);       // [n]
-    GRIDFF_CUDA(cudaMemcpyAsync(d_coef, h_coef, (size_t)n * 16, cudaMemcpyHostToDevice, st));
-    GRIDFF_CUDA(cudaMemcpyAsync(d_pos, h_pos, (size_t)n * 12, cudaMemcpyHostToDevice, st));
-    int rc = gridff_eval(grid, n, d_pos, d_coef, h_E ? d_E : nullptr, h_F ? d_F : nullptr, cuda_stream);
-    if (rc) return rc;
-    if (h_E) GRIDFF_CUDA(cudaMemcpyAsync(h_E, d_E, (size_t)n * 4, cudaMemcpyDeviceToHost, st));
-    if (h_F) GRIDFF_CUDA(cudaMemcpyAsync(h_F, d_F, (size_t)n * 12, cudaMemcpyDeviceToHost, st));
+    // Pipelined in chunks over three streams so that, with pinned host buffers, the upload of chunk c+1, the kernel of chunk c and the
+    // download of chunk c-1 overlap (PCIe is full duplex): the call is then bound by max(upload, download), not by their sum.
+    static thread_local cudaStream_t s_in = nullptr, s_out = nullptr;
+    static thread_local cudaEvent_t ev_start = nullptr, ev_in[2] = {nullptr, nullptr}, ev_k[2] = {nullptr, nullptr}, ev_out = nullptr;
+    if (!s_in) {
+        GRIDFF_CUDA(cudaStreamCreateWithFlags(&s_in, cudaStreamNonBlocking));
+        GRIDFF_CUDA(cudaStreamCreateWithFlags(&s_out, cudaStreamNonBlocking));
+        GRIDFF_CUDA(cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming));
+        GRIDFF_CUDA(cudaEventCreateWithFlags(&ev_out, cudaEventDisableTiming));
+        for (int k = 0; k < 2; ++k) {
+            GRIDFF_CUDA(cudaEventCreateWithFlags(&ev_in[k], cudaEventDisableTiming));
+            GRIDFF_CUDA(cudaEventCreateWithFlags(&ev_k[k], cudaEventDisableTiming));
+        }
+    }
+    const long long chunk = 1ll << 22;                  // 4 Mi points: 117 MB up, 67 MB down per chunk
+    GRIDFF_CUDA(cudaEventRecord(ev_start, st));         // work already enqueued on the caller's stream (e.g. the grid build) comes first
+    GRIDFF_CUDA(cudaStreamWaitEvent(s_in, ev_start, 0));
+    GRIDFF_CUDA(cudaStreamWaitEvent(s_out, ev_start, 0));
+    int c = 0;
+    for (long long p0 = 0; p0 < n; p0 += chunk, ++c) {
+        const long long m = n - p0 < chunk ? n - p0 : chunk;
+        const int k = c & 1;
+        GRIDFF_CUDA(cudaMemcpyAsync(d_coef + 4 * p0, h_coef + 4 * p0, (size_t)m * 16, cudaMemcpyHostToDevice, s_in));
+        GRIDFF_CUDA(cudaMemcpyAsync(d_pos + 3 * p0, h_pos + 3 * p0, (size_t)m * 12, cudaMemcpyHostToDevice, s_in));
+        GRIDFF_CUDA(cudaEventRecord(ev_in[k], s_in));
+        GRIDFF_CUDA(cudaStreamWaitEvent(st, ev_in[k], 0));
+        int rc = gridff_eval(grid, m, d_pos + 3 * p0, d_coef + 4 * p0, h_E ? d_E + p0 : nullptr, h_F ? d_F + 3 * p0 : nullptr, cuda_stream);
+        if (rc) return rc;
+        GRIDFF_CUDA(cudaEventRecord(ev_k[k], st));
+        GRIDFF_CUDA(cudaStreamWaitEvent(s_out, ev_k[k], 0));
+        if (h_E) GRIDFF_CUDA(cudaMemcpyAsync(h_E + p0, d_E + p0, (size_t)m * 4, cudaMemcpyDeviceToHost, s_out));
+        if (h_F) GRIDFF_CUDA(cudaMemcpyAsync(h_F + 3 * p0, d_F + 3 * p0, (size_t)m * 12, cudaMemcpyDeviceToHost, s_out));
+    }
+    GRIDFF_CUDA(cudaEventRecord(ev_out, s_out));
+    GRIDFF_CUDA(cudaStreamWaitEvent(st, ev_out, 0));
     GRIDFF_CUDA(cudaStreamSynchronize(st));
     return GRIDFF_OK;
 }
