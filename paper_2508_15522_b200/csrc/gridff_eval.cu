@@ -36,10 +36,22 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
     s_base[w][lane] = s.base; s_cf[w][lane] = cf;
     __syncwarp();
     float* tile = s_tile[w];
+    // do this warp's points share stencils?  (spatially sorted input: most lanes sit in their neighbour's cell)  Then the L1 pays;
+    // otherwise gather past it
+    const unsigned prev = __shfl_up_sync(0xFFFFFFFFu, s.base, 1);
+    const bool clustered = __popc(__ballot_sync(0xFFFFFFFFu, lane > 0 && prev == s.base)) >= 8;
+    if (clustered) {
 #pragma unroll 8
-    for (int q = 0; q < 32; ++q) {
-        const unsigned b = s_base[w][q];
-        if (b != kNoStencil) gather_rows(g, b, s_cf[w][q], lane, q, tile);
+        for (int q = 0; q < 32; ++q) {
+            const unsigned b = s_base[w][q];
+            if (b != kNoStencil) gather_rows<false>(g, b, s_cf[w][q], lane, q, tile);
+        }
+    } else {
+#pragma unroll 8
+        for (int q = 0; q < 32; ++q) {
+            const unsigned b = s_base[w][q];
+            if (b != kNoStencil) gather_rows<true>(g, b, s_cf[w][q], lane, q, tile);
+        }
     }
     __syncwarp();
     if (p >= n) return;
