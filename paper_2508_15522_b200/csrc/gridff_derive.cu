@@ -48,12 +48,15 @@ __global__ void __launch_bounds__(kWarps * 32) k_eval_half(GridGeom g, long long
     const int k = lane & 3, r0 = lane >> 2;
     const int rs = g.nzp, ps = g.sy * g.nzp;
     const int off = (r0 >> 2) * ps + (r0 & 3) * rs + k;
+    // per-warp load path as in k_eval_coop: through the L1 when the warp's points share cells, past it otherwise
+    const unsigned prev = __shfl_up_sync(0xFFFFFFFFu, s.base, 1);
+    const bool clustered = __popc(__ballot_sync(0xFFFFFFFFu, lane > 0 && prev == s.base)) >= 8;
 #pragma unroll 8
     for (int q = 0; q < 32; ++q) {
         const unsigned b = s_base[w][q];
         if (b != kNoStencil) {
             const uint2* a = store + b + off;
-            const uint2 n0 = __ldg(a), n1 = __ldg(a + 2 * ps);
+            const uint2 n0 = clustered ? __ldg(a) : __ldcg(a), n1 = clustered ? __ldg(a + 2 * ps) : __ldcg(a + 2 * ps);
             const float4 c = s_cf[w][q];
             tile[tile_word(q, lane)] = fold_half(c, n0);
             tile[tile_word(q, lane + 32)] = fold_half(c, n1);
