@@ -119,3 +119,21 @@ def test_defective_substrate_grid_and_eval(api, orc):
     p2 = np.array([[v0[0], v0[1], 2.0], [(v0[0] + 2 * 2.82) % Lx, v0[1], 2.0]])
     V = orc.interp(og, p2, np.array([[1.0, 0, 0, 0]] * 2))[0]
     assert abs(V[0] - V[1]) > 1e-3 * abs(V[1])
+
+
+def test_morse_window_is_exact(api, orc, cfg1s, monkeypatch):
+    """The magnitude-window Morse sampling (terms more than e^-46 below a node's largest term skipped; used for large image blocks such
+    as config 3's) must give the same fp32 coefficients as the full sum, and the oracle's."""
+    og, _ = oracle_grid(orc, cfg1s["sub"], cfg1s["desc"])
+    out = {}
+    for flag in ("0", "1"):
+        monkeypatch.setenv("GRIDFF_MORSE_WINDOW", flag)
+        g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
+        out[flag] = api.gridff_grid_export(g).cpu().numpy()
+    assert np.array_equal(out["0"][..., 2], out["1"][..., 2])                  # Coulomb untouched
+    d = np.abs(out["0"].astype(np.float64) - out["1"])
+    assert np.all(d <= 6e-8 * np.abs(out["0"]) + 1e-12 * np.abs(out["0"]).max())         # at most the last fp32 bit
+    assert (d > 0).mean() < 1e-3
+    for c in range(2):
+        ref = og.coef[..., c]
+        assert np.all(np.abs(out["1"][..., c] - ref) <= 6.0e-8 * np.abs(ref) + 1e-9 * np.abs(ref).max())
