@@ -4,8 +4,15 @@ TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and b
 cpu_baseline / --impl reference legs may import this.  It imports nothing from
 paper_2508_15522_b200 and shares no code with the CUDA path.
 
-Argument marshalling only; all arithmetic is in the C file.  Inputs are widened to float64
-exactly (the GPU path receives the same values as float32).
+Argument marshalling for the C file, which holds the arithmetic of the hot path (pins listed in its header), plus — written here in
+plain numpy / Python loops, fp64 — the SURVEY.md §8(f) pieces that are definitions rather than numerics:
+  same_structure, unique_filter     PAPER.md:L241 criterion (R16), sequential greedy filter
+                                    pinned: constructed populations collapse to the known K structures; brute-force invariants
+  minima_hopping                    PAPER.md:L222 loop composed of the pinned Langevin / FIRE calls and the filter (R19)
+                                    pinned: records are minima, pairwise distinct; 2 cycles == 1 + 1 cycles
+  half_grid                         fp64 -> fp32 -> fp16 coefficient rounding (numpy's IEEE casts)       pinned: 2^-11 bound
+  trilinear_nodes, interp_trilinear PAPER.md:L118-120 foil (R20)    pinned: scipy RegularGridInterpolator, exact at nodes
+Inputs are widened to float64 exactly (the GPU path receives the same values as float32).
 """
 import ctypes as C
 import os
