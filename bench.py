@@ -68,7 +68,7 @@ def workload(args):
 
 # ------------------------------------------------------------------------------------------------------------------ oracle arm
 
-def oracle_sample(cfg, md_steps, n_rep_sample=64, steps_sample=200):
+def oracle_sample(cfg, md_steps, n_rep_sample=512, steps_sample=1000):
     """Times the fp64 oracle, as it stands, on a bounded sample: the whole grid build (a1-a3) + n_rep_sample replicas x
     steps_sample steps (a5-a9).  Returns (t_build, t_per_replica_step, cores)."""
     from oracle import gridff_oracle as orc
