@@ -26,7 +26,9 @@
  *                    variance of free particles, equipartition, normal moments  pinned
  *   held atoms/scan  one-atom scan = the interpolated potential itself;
  *                    held atoms never move; relaxed E <= unrelaxed E            pinned
- *   basin assignment parity unpinned (only oracle-vs-GPU agreement exists)
+ *   basin assignment parity unpinned: WHICH minimum a given start relaxes to has no external reference (only
+ *                    oracle-vs-GPU agreement); that the end state IS a minimum (max |F_i| < f_tol, E <= E_start) and the
+ *                    same-structure criterion itself (gridff_oracle.py same_structure) are pinned
  */
 #include <math.h>
 #include <stdint.h>
