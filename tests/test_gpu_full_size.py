@@ -132,3 +132,29 @@ def test_config3_full_size_properties(api, orc):
     r0 = run_gpu(api, g, mol, api.make_integrator("vv", 0, 0.5), cfg["pos"], cfg["vel"])
     e0, e1 = r0["energy"].astype(np.float64).sum(1), r3["energy"].astype(np.float64).sum(1)
     assert np.all(np.abs(e1 - e0) <= 0.05 * r0["energy"][:, 7] + 2e-3)
+
+
+@pytest.mark.parametrize("kind", ["vv", "langevin"])
+def test_config1_time_multiplexed_launch_is_bit_identical(api, kind):
+    """The bench's launch shape (4096 replicas, >= 512 steps) runs the fixed-length integrators time-multiplexed: each block owns 14
+    replicas and cycles them over its 8 warps in 8 chunks of steps, the state passing through the pos / vel arrays between rounds.
+    It must equal, bit for bit, eight short launches (80 steps each: below the multiplexing threshold, one replica per warp) — which in
+    turn are compared with the oracle in test_config1_full_grid_sampled_replicas and test_langevin_trajectory_100_steps."""
+    cfg = inputs.config(1)
+    g = gpu_grid(api, cfg["sub"], cfg["desc"], l2_persist=1)
+    mol = gpu_side(api, cfg)
+    kw = dict(temperature=300.0, gamma=0.01, seed=11) if kind == "langevin" else {}
+    one = run_gpu(api, g, mol, api.make_integrator(kind, 640, 0.5, **kw), cfg["pos"], cfg["vel"])
+    p, v = cfg["pos"], cfg["vel"]
+    for b in range(8):
+        kw_b = dict(kw, step0=80 * b) if kind == "langevin" else kw
+        r = run_gpu(api, g, mol, api.make_integrator(kind, 80, 0.5, **kw_b), p, v)
+        p, v = r["pos"], r["vel"]
+    assert np.array_equal(one["pos"], p) and np.array_equal(one["vel"], v)
+    assert np.array_equal(one["energy"], r["energy"])
+    assert np.all(one["status"][:, 0] == 640) and np.all(np.isfinite(one["pos"]))
+    # ragged replica counts: a last block with fewer replicas than warps, and one with more
+    for n_rep in (2369, 4001):
+        a = run_gpu(api, g, mol, api.make_integrator(kind, 520, 0.5, **kw), cfg["pos"][:n_rep], cfg["vel"][:n_rep])
+        assert np.array_equal(a["pos"][:64], run_gpu(api, g, mol, api.make_integrator(kind, 520, 0.5, **kw), cfg["pos"][:64], cfg["vel"][:64])["pos"])
+        assert np.all(np.isfinite(a["pos"])) and np.all(a["status"][:, 0] == 520)
