@@ -158,3 +158,21 @@ def test_config1_time_multiplexed_launch_is_bit_identical(api, kind):
         a = run_gpu(api, g, mol, api.make_integrator(kind, 520, 0.5, **kw), cfg["pos"][:n_rep], cfg["vel"][:n_rep])
         assert np.array_equal(a["pos"][:64], run_gpu(api, g, mol, api.make_integrator(kind, 520, 0.5, **kw), cfg["pos"][:64], cfg["vel"][:64])["pos"])
         assert np.all(np.isfinite(a["pos"])) and np.all(a["status"][:, 0] == 520)
+
+
+def test_time_multiplexed_two_atoms_per_lane(api):
+    """the same bit-identity for a molecule above 32 atoms (one block of 8 warps per SM): 1400 replicas of a 40-atom chain"""
+    from gridff_cases import small_config
+    cfg = small_config(1, n_rep=1)
+    d = cfg["desc"]
+    g = gpu_grid(api, cfg["sub"], d)
+    topo = inputs.helix_chain(40, seed=3)
+    mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
+    pos = inputs.place_replicas(topo, 1400, d["Lx"], d["Ly"], 0.0, 5)
+    vel = inputs.maxwell_boltzmann(topo, 1400, 300.0, 6)
+    one = run_gpu(api, g, mol, api.make_integrator("vv", 560, 0.5), pos, vel)
+    p, v = pos, vel
+    for _ in range(7):
+        r = run_gpu(api, g, mol, api.make_integrator("vv", 80, 0.5), p, v)
+        p, v = r["pos"], r["vel"]
+    assert np.array_equal(one["pos"], p) and np.array_equal(one["vel"], v) and np.array_equal(one["energy"], r["energy"])
