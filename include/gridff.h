@@ -175,7 +175,9 @@ typedef struct {
     unsigned long long seed;
     float z_ref, place_z_lo, place_z_hi, place_z_min, clash;   /* restart placement (3, 6, 2 Å above z_ref; clash factor 0.4) */
     int variant;              /* kernel variant: 0 = default (library's choice), 1 = one thread per atom gathers its 64 nodes, 2 = warp-cooperative row gather every step,
-                                 3 = 2 + the folded stencils cached in shared memory and re-gathered only when an atom changes cell */
+                                 3 = 2 + the folded stencils cached in shared memory and re-gathered only when an atom changes cell.
+                                 Molecules of 33-64 atoms: variants 1, 2 put two atoms on a lane; variant 3 puts the replica on a pair of warps
+                                 (one atom per lane).  All variants compute the same forces; they differ in rounding order only. */
     /* SURVEY.md §8(f) rows 1-2 (0 / unset = off) */
     float temperature;        /* K, kind 2 */
     float gamma;              /* friction 1/fs, kind 2: per step  B: v += dt/2 a;  A: x += dt/2 v;  O: v = c1 v + c2 sqrt(kT/m) xi;  A;  F(x);  B,
