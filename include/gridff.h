@@ -66,6 +66,8 @@ typedef struct {
     int channel[4];       /* gridff_channel per stored component                                                        */
     int layout;           /* gridff_layout                                                                              */
     int l2_persist;       /* 1: ask for an L2 access-policy window over the store on the streams that use the grid      */
+    int morse_window;     /* Morse sampling (a1): 0 = library's choice, 1 = always skip the terms below fp64 rounding of the node's
+                             sum (the magnitude window), 2 = never (every image term is evaluated); same coefficients  */
 } gridff_grid_desc;
 
 /* nodes per axis, spacings and origin {0, 0, z_ref+z_lo} implied by a descriptor. */
@@ -78,8 +80,10 @@ int gridff_grid_bytes(const gridff_grid_desc* desc, int n_sub, size_t* store_byt
 /* Sample the channels on the grid, prefilter them to interpolating cubic B-spline coefficients (cyclic in x,y;
  * not-a-knot in z) and write the interleaved fp32 store.
  *   sub_pos [n_sub][3], sub_e (sqrt(eps_j), eV^1/2), sub_R (Å), sub_q (e): HOST doubles; sub_q may be NULL without a
- *   Coulomb channel.  A Coulomb channel needs |sum q| < 1e-9 e (GRIDFF_EUNSUPPORTED otherwise) and a grid that starts
- *   above every substrate atom.  Sampling and prefilter run in fp64 on the device; the store is fp32.
+ *   Coulomb channel.  A Coulomb channel needs |sum q| < 1e-9 e (GRIDFF_EUNSUPPORTED otherwise) and z_ref at or above the
+ *   topmost substrate atom (an adatom or a step included: z_ref is THEIR z; GRIDFF_EINVAL otherwise), so that the lowest
+ *   grid plane lies at least z_lo > 0 above every atom — the Fourier sum is cut where exp(-|G| z_lo) < 1e-16.
+ *   Sampling and prefilter run in fp64 on the device; the store is fp32.
  *   Synchronises the stream once (host -> device copy of the substrate from pageable memory).                    */
 int gridff_build_grid(const gridff_grid_desc* desc, int n_sub,
                       const double* sub_pos, const double* sub_e, const double* sub_R, const double* sub_q,
@@ -153,7 +157,7 @@ typedef struct {
     /* restart generator (used with integrator.restart = 1) */
     int n_rot; const int* rot_bond;                /* [.][2] rotatable bonds j0 -> j1 */
     const unsigned char* rot_mask;                 /* [.][n] 1 = atom turns with j1 */
-    const float* ref_pos;                          /* [n][3] template conformation */
+    const float* ref_pos;                          /* [n][3] template conformation; required by integrator.restart = 1 (GRIDFF_EINVAL without it) */
 } gridff_topology;                                 /* HOST arrays; copied by gridff_create_molecule */
 
 typedef struct gridff_molecule gridff_molecule;
@@ -177,7 +181,9 @@ typedef struct {
     int variant;              /* kernel variant: 0 = default (library's choice), 1 = one thread per atom gathers its 64 nodes, 2 = warp-cooperative row gather every step,
                                  3 = 2 + the folded stencils cached in shared memory and re-gathered only when an atom changes cell.
                                  Molecules of 33-64 atoms: variants 1, 2 put two atoms on a lane; variant 3 puts the replica on a pair of warps
-                                 (one atom per lane).  All variants compute the same forces; they differ in rounding order only. */
+                                 (one atom per lane); variant 4 = variant 3's stencil cache on ONE warp with two atoms per lane (the older kernel, kept
+                                 for the design comparison; for <= 32 atoms it is variant 3).  All variants compute the same forces; they differ in
+                                 rounding order only. */
     /* SURVEY.md §8(f) rows 1-2 (0 / unset = off) */
     float temperature;        /* K, kind 2 */
     float gamma;              /* friction 1/fs, kind 2: per step  B: v += dt/2 a;  A: x += dt/2 v;  O: v = c1 v + c2 sqrt(kT/m) xi;  A;  F(x);  B,
@@ -194,7 +200,8 @@ typedef struct {
  * round-trips: per step, grid forces by interpolation + intramolecular terms + integrator.
  *   d_pos, d_vel   [n_rep][n][3]  in/out, fp32
  *   d_fire         [n_rep][4]     in/out FIRE scalars {dt, a, steps since P<=0, restarts done}; dt <= 0 = fresh.  May be NULL (VV, or fresh FIRE)
- *   d_energy       [n_rep][8]     out: grid ch0, ch1, ch2, bond, angle, torsion, non-bonded, kinetic (eV) at the final state.  May be NULL
+ *   d_energy       [n_rep][8]     out: grid ch0, ch1, ch2 (+ ch3 when the grid has a 4th channel), bond, angle, torsion, non-bonded, kinetic (eV)
+ *                                 at the final state: the first 7 sum to the potential whose gradient the forces are.  May be NULL
  *   d_status       [n_rep][2]     out: {steps taken, converged flag (restart=0) or minima recorded (restart=1)}.  May be NULL
  *   d_minima       [cap][4+3n]    out, restart=1: {replica, restart#, steps, E_total, positions}; d_n_minima (1 int, device, caller zeroes it)
  *                                 counts records (may exceed cap; excess dropped).  May be NULL

@@ -472,7 +472,8 @@ void orc_intramolecular(const orc_topology* T, const double* pos, double* F, dou
 }
 
 /* Total force and the 7 potential-energy terms of one replica:
- * E7 = {grid ch0, grid ch1, grid ch2, bond, angle, torsion, non-bonded}.   */
+ * E7 = {grid ch0, grid ch1, grid ch2 (+ ch3 if the grid has a 4th channel), bond, angle, torsion, non-bonded}: the 7 terms sum to the
+ * potential whose gradient F is (R22; the paper has three channels).   */
 void orc_forces(const orc_grid* g, const orc_topology* T, const double* pos, double* F, double* E7) {
     int n = T->n_atoms;
     for (int i = 0; i < 3 * n; ++i) F[i] = 0;
@@ -482,7 +483,7 @@ void orc_forces(const orc_grid* g, const orc_topology* T, const double* pos, dou
         interp_point(g, pos + 3 * i, V, dV);
         for (int c = 0; c < g->nch; ++c) {
             double k = T->coef[4 * i + c];
-            if (c < 3) E7[c] += k * V[c];
+            E7[c < 3 ? c : 2] += k * V[c];
             for (int d = 0; d < 3; ++d) F[3 * i + d] -= k * dV[3 * c + d];
         }
     }

@@ -35,7 +35,7 @@ class GridffError(RuntimeError):
 class GridDesc(C.Structure):
     _fields_ = [("Lx", C.c_double), ("Ly", C.c_double), ("z_ref", C.c_double), ("z_lo", C.c_double), ("z_hi", C.c_double),
                 ("spacing", C.c_double), ("alpha", C.c_double), ("r_cut", C.c_double),
-                ("n_channels", C.c_int), ("channel", C.c_int * 4), ("layout", C.c_int), ("l2_persist", C.c_int)]
+                ("n_channels", C.c_int), ("channel", C.c_int * 4), ("layout", C.c_int), ("l2_persist", C.c_int), ("morse_window", C.c_int)]
 
 
 class Topology(C.Structure):
@@ -140,13 +140,13 @@ def _hptr(a):
     return None if a is None else C.c_void_p(a.ctypes.data)
 
 
-def make_desc(Lx, Ly, z_ref, z_lo, z_hi, spacing, alpha, channels, r_cut=17.0, layout=LAYOUT_ZFAST, l2_persist=0):
+def make_desc(Lx, Ly, z_ref, z_lo, z_hi, spacing, alpha, channels, r_cut=17.0, layout=LAYOUT_ZFAST, l2_persist=0, morse_window=0):
     d = GridDesc()
     d.Lx, d.Ly, d.z_ref, d.z_lo, d.z_hi, d.spacing, d.alpha, d.r_cut = Lx, Ly, z_ref, z_lo, z_hi, spacing, alpha, r_cut
     d.n_channels = len(channels)
     for k in range(4):
         d.channel[k] = int(channels[k]) if k < len(channels) else CH_ZERO
-    d.layout, d.l2_persist = int(layout), int(l2_persist)
+    d.layout, d.l2_persist, d.morse_window = int(layout), int(l2_persist), int(morse_window)
     return d
 
 

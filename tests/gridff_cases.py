@@ -19,13 +19,13 @@ def oracle_grid(orc, sub, desc):
     return _ORACLE_GRIDS[key]
 
 
-def gpu_desc(api, desc, layout=0, l2_persist=0):
+def gpu_desc(api, desc, layout=0, l2_persist=0, morse_window=0):
     return api.make_desc(desc["Lx"], desc["Ly"], desc["z_ref"], desc["z_lo"], desc["z_hi"], desc["spacing"], desc["alpha"],
-                         desc["channels"], r_cut=desc["r_cut"], layout=layout, l2_persist=l2_persist)
+                         desc["channels"], r_cut=desc["r_cut"], layout=layout, l2_persist=l2_persist, morse_window=morse_window)
 
 
-def gpu_grid(api, sub, desc, layout=0, l2_persist=0):
-    d = gpu_desc(api, desc, layout, l2_persist)
+def gpu_grid(api, sub, desc, layout=0, l2_persist=0, morse_window=0):
+    d = gpu_desc(api, desc, layout, l2_persist, morse_window)
     return api.gridff_build_grid(d, sub["pos"], sub["e"], sub["R"], sub["q"])
 
 

@@ -197,22 +197,21 @@ def test_vv_trajectory_100_steps(api, orc, k, variant):
 
 
 @pytest.mark.parametrize("k", [1, 2])
-def test_stencil_cache_is_bit_identical(api, k, monkeypatch):
+def test_stencil_cache_is_bit_identical(api, k):
     """variant 3 (folded stencils cached, re-gathered on cell change) computes exactly what variant 2 (gather every step) does.  (For the
-    60-atom molecule the comparison is between the two one-warp kernels; the default pair-of-warps kernel sums the same forces in another
-    order and is compared with the oracle and, to rounding, with these in test_pair_of_warps_kernel_matches_one_warp_kernel.)"""
-    if k == 2:
-        monkeypatch.setenv("GRIDFF_TWO_ATOMS_PER_LANE", "1")
+    60-atom molecule the comparison is between the two one-warp kernels, variants 2 and 4; the default pair-of-warps kernel sums the same
+    forces in another order and is compared with the oracle and, to rounding, with these in test_pair_of_warps_kernel_matches_one_warp_kernel.)"""
+    cached = 4 if k == 2 else 3
     cfg = small_config(k, n_rep=41)
     g = gpu_grid(api, cfg["sub"], cfg["desc"])
     mol = gpu_side(api, cfg)
     vel = inputs.maxwell_boltzmann(cfg["topo"], 41, 600.0, 17)
     r2 = run_gpu(api, g, mol, api.make_integrator("vv", 400, 0.5, variant=2), cfg["pos"], vel)
-    r3 = run_gpu(api, g, mol, api.make_integrator("vv", 400, 0.5, variant=3), cfg["pos"], vel)
+    r3 = run_gpu(api, g, mol, api.make_integrator("vv", 400, 0.5, variant=cached), cfg["pos"], vel)
     assert np.array_equal(r2["pos"], r3["pos"]) and np.array_equal(r2["vel"], r3["vel"]) and np.array_equal(r2["energy"], r3["energy"])
 
 
-def test_pair_of_warps_kernel_matches_one_warp_kernel(api, orc, monkeypatch):
+def test_pair_of_warps_kernel_matches_one_warp_kernel(api, orc):
     """60-atom molecule: the default kernel (replica on a pair of warps, one atom per lane) against the one-warp kernel (two atoms per lane):
     velocity Verlet, FIRE with restart and Langevin agree to rounding over 40 steps, energies to 1e-5 relative"""
     cfg = small_config(2, n_rep=23)
@@ -220,12 +219,10 @@ def test_pair_of_warps_kernel_matches_one_warp_kernel(api, orc, monkeypatch):
     mol = gpu_side(api, cfg)
     vel = inputs.maxwell_boltzmann(cfg["topo"], 23, 300.0, 19)
     runs = {}
-    for flag in ("0", "1"):
-        if flag == "1":
-            monkeypatch.setenv("GRIDFF_TWO_ATOMS_PER_LANE", "1")
-        runs[flag] = [run_gpu(api, g, mol, api.make_integrator("vv", 40, 0.5), cfg["pos"], vel),
-                      run_gpu(api, g, mol, api.make_integrator("langevin", 40, 0.5, temperature=300.0, gamma=0.01, seed=3), cfg["pos"], vel),
-                      run_gpu(api, g, mol, api.make_integrator("fire", 40, 0.5, f_tol=1e-6), cfg["pos"], np.zeros_like(vel), fire=np.zeros((23, 4), np.float32))]
+    for flag, v in (("0", 3), ("1", 4)):              # variant 3 = pair of warps, 4 = one warp with two atoms per lane (gridff.h)
+        runs[flag] = [run_gpu(api, g, mol, api.make_integrator("vv", 40, 0.5, variant=v), cfg["pos"], vel),
+                      run_gpu(api, g, mol, api.make_integrator("langevin", 40, 0.5, temperature=300.0, gamma=0.01, seed=3, variant=v), cfg["pos"], vel),
+                      run_gpu(api, g, mol, api.make_integrator("fire", 40, 0.5, f_tol=1e-6, variant=v), cfg["pos"], np.zeros_like(vel), fire=np.zeros((23, 4), np.float32))]
     for a, b in zip(runs["0"], runs["1"]):
         assert np.abs(a["pos"] - b["pos"]).max() <= 5e-5 and np.abs(a["vel"] - b["vel"]).max() <= 1e-5
         check_energies(a["energy"], b["energy"].astype(np.float64), tol_rel=2e-5, tol_abs=2e-5)

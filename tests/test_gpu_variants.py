@@ -121,14 +121,13 @@ def test_defective_substrate_grid_and_eval(api, orc):
     assert abs(V[0] - V[1]) > 1e-3 * abs(V[1])
 
 
-def test_morse_window_is_exact(api, orc, cfg1s, monkeypatch):
+def test_morse_window_is_exact(api, orc, cfg1s):
     """The magnitude-window Morse sampling (terms more than e^-46 below a node's largest term skipped; used for large image blocks such
     as config 3's) must give the same fp32 coefficients as the full sum, and the oracle's."""
     og, _ = oracle_grid(orc, cfg1s["sub"], cfg1s["desc"])
     out = {}
-    for flag in ("0", "1"):
-        monkeypatch.setenv("GRIDFF_MORSE_WINDOW", flag)
-        g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
+    for flag, mw in (("0", 2), ("1", 1)):                    # gridff_grid_desc.morse_window: 2 = never, 1 = always
+        g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"], morse_window=mw)
         out[flag] = api.gridff_grid_export(g).cpu().numpy()
     assert np.array_equal(out["0"][..., 2], out["1"][..., 2])                  # Coulomb untouched
     d = np.abs(out["0"].astype(np.float64) - out["1"])
