@@ -1,0 +1,235 @@
+"""FIRE relaxation, restarts and basin assignment: GPU fp32 path against the fp64 oracle (run on the B200 box with -m gpu).
+
+north_star asks for "identical minimum-energy basin assignment for relaxed replicas".  Three kinds of statement are tested here:
+
+ 1. WELL-POSED cases must match 100 %: from starts near a minimum (an oracle minimum displaced by 0.02 Å) both sides must converge
+    and land in the SAME basin, every replica.
+ 2. FAR-FROM-MINIMUM starts (the configs as stated: random placements 3-6 Å above the surface) are chaotic: FIRE takes a discrete
+    decision per step (P = F.v > 0 ?), and one decision taken a step apart changes dt for the rest of the run.  The CONTROL is the fp64
+    oracle itself advanced one step per call with its state (positions, velocities, FIRE scalars) rounded to fp32 between calls — exact
+    forces, the storage precision of the GPU path (`control_run`; the oracle's launch-split invariance is one of its pins).  It does not
+    reproduce the plain fp64 run in every replica.  That rate m0 is MEASURED in the same test, printed, and the GPU-vs-oracle
+    mismatch must not exceed it by more than a binomial margin (gridff_cases.chaos_margin).  There is no fixed 50-90 % bar any more.
+ 3. What is unique regardless of chaos: every minimum the GPU reports satisfies the convergence criterion under the ORACLE's forces,
+    carries the oracle's energy for that state, and the oracle's tight re-relaxation from it converges downhill to a minimum.
+
+Basin identity is PAPER.md:L241's criterion (R16) applied to POLISHED states: the basin of a state is the minimum the oracle's
+FIRE (to 2e-5 eV/Å) flows to from it — the same polish for both sides.  The configs' own tolerance (1e-3 eV/Å) does not define a
+structure to the 0.1 Å of the criterion: measured with the oracle on config 0, states that satisfy max |F_i| < 1e-3 eV/Å lie 0.1 ... 2.5 Å
+RMSD (median 0.5 Å) and up to 0.09 eV from the minimum they flow to (benzene sliding over the weakly corrugated surface), while polished
+states are reproducible to 0.016 Å / 1e-6 eV (2e-5 against 2e-6 eV/Å).  The 48 config-0 starts have two distinct polished minima.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2508_15522_b200 import inputs
+from gridff_cases import oracle_grid, gpu_grid, small_config, basin_match, chaos_margin, energy_scales
+from test_gpu_parity import api, dev, oracle_side, gpu_side, run_gpu, check_energies, TRAJ_TOL  # noqa: F401
+
+pytestmark = pytest.mark.gpu
+
+_CONTROLS = {}
+
+
+def control_run(orc, og, ot, make_integ, n_steps, pos, vel, minima_cap=0, key=None):
+    """The chaos control: the fp64 oracle, one step per call, state rounded to fp32 between calls.  `make_integ(n)` builds the oracle
+    integrator for n steps.  Returns what orc.run_replicas returns (status[:, 0] = total steps taken, minima accumulated over the calls)."""
+    if key is not None and key in _CONTROLS:
+        return _CONTROLS[key]
+    p, v = np.asarray(pos, np.float32), np.asarray(vel, np.float32)
+    f = np.zeros((len(p), 4), np.float32)
+    integ = make_integ(1)
+    steps = np.zeros(len(p), np.int64); minima = []
+    for _ in range(n_steps):
+        o = orc.run_replicas(og, ot, integ, p, v, fire=f, minima_cap=minima_cap)
+        p, v, f = o["pos"].astype(np.float32), o["vel"].astype(np.float32), o["fire"].astype(np.float32)
+        steps += o["status"][:, 0]
+        if minima_cap:
+            minima.extend(o["minima"])
+    out = dict(o, status=np.stack([steps, o["status"][:, 1]], 1), minima=np.array(minima).reshape(len(minima), 4 + 3 * p.shape[1]), n_minima=len(minima))
+    if key is not None:
+        _CONTROLS[key] = out
+    return out
+
+
+def polish(orc, og, ot, x, f_tol=2e-5, steps=400000):
+    """oracle FIRE from rest to a tight tolerance: -> (E, x, converged).  (With real masses FIRE needs ~4e4 iterations to go from 1e-3 to
+    2e-5 eV/Å on these soft adsorbates, R13: a few seconds of oracle time per batch.)"""
+    x = np.asarray(x, np.float64)
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", steps, 1.0, f_tol=f_tol, dt_max=20.0, max_step=0.1), x, np.zeros_like(x))
+    return o["energy"][:, :7].sum(1), o["pos"], o["status"][:, 1] == 1
+
+
+def assert_true_minima(orc, og, ot, x, E_reported, f_tol, what):
+    """statement 3 of the module docstring for the states x [m][n][3] with reported total energies E_reported; returns the polished (E, x)"""
+    x = np.asarray(x, np.float64)
+    for k in range(len(x)):
+        E7, F = orc.forces(og, ot, x[k])
+        assert np.sqrt((F ** 2).sum(1)).max() < 1.05 * f_tol, (what, k)
+        scale = np.abs(E7).sum()
+        assert abs(E_reported[k] - E7.sum()) <= 2e-5 * scale + 2e-5, (what, k, E_reported[k], E7.sum())
+    Ep, xp, conv = polish(orc, og, ot, x)
+    # (the 60-atom chain's softest torsional modes can take more than the polish's 4e5 iterations to reach 2e-5 eV/Å: those are still flowing downhill)
+    assert conv.mean() >= 0.7, (what, "polish did not converge", conv.sum(), len(conv))
+    assert np.all(Ep <= np.asarray(E_reported, np.float64) + 1e-5), (what, "polish went uphill")
+    return Ep, xp
+
+
+def basins(orc, og, ot, o, key=None):
+    """polished (E, x, converged) of the end states of a run (cached for the oracle-side runs that several parametrised tests share)"""
+    if key is not None and key in _CONTROLS:
+        return _CONTROLS[key]
+    out = polish(orc, og, ot, o["pos"])
+    if key is not None:
+        _CONTROLS[key] = out
+    return out
+
+
+def test_fire_first_steps_and_launch_split(api, orc):
+    """FIRE: 1 x 200 steps == 4 x 50 steps bit for bit when the FIRE scalars are carried.  Trajectories: N FIRE steps against the oracle for
+    N = 30, 100, 300.  A replica whose decision history equals the oracle's (same dt, a and step counter at the end) on the GPU AND in the
+    control MUST be within the trajectory tolerance 1e-3 Å; the number of replicas whose history differs must not exceed the control's."""
+    cfg = small_config(0, n_rep=21)
+    og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
+    g = gpu_grid(api, cfg["sub"], cfg["desc"])
+    ot, mol = oracle_side(orc, cfg, og), gpu_side(api, cfg)
+    vel = np.zeros_like(cfg["pos"]); fire0 = np.zeros((21, 4), np.float32)
+    r1 = run_gpu(api, g, mol, api.make_integrator("fire", 200, 0.5, f_tol=1e-6), cfg["pos"], vel, fire=fire0)
+    p, v, f = cfg["pos"], vel, fire0
+    for _ in range(4):
+        r4 = run_gpu(api, g, mol, api.make_integrator("fire", 50, 0.5, f_tol=1e-6), p, v, fire=f)
+        p, v, f = r4["pos"], r4["vel"], r4["fire"]
+    assert np.array_equal(r1["pos"], r4["pos"]) and np.array_equal(r1["fire"], r4["fire"])
+    report = {}
+    for N in (30, 100, 300):
+        r = run_gpu(api, g, mol, api.make_integrator("fire", N, 0.5, f_tol=1e-6), cfg["pos"], vel, fire=fire0)
+        o = orc.run_replicas(og, ot, orc.make_integrator("fire", N, 0.5, f_tol=1e-6), cfg["pos"], vel)
+        c = control_run(orc, og, ot, lambda n: orc.make_integrator("fire", n, 0.5, f_tol=1e-6), N, cfg["pos"], vel)
+        same_hist = lambda a: np.all(np.isclose(a["fire"][:, :3], o["fire"][:, :3], rtol=1e-5), axis=1)
+        hist, hist_c = same_hist(r), same_hist(c)
+        dev_g = np.abs(r["pos"].astype(np.float64) - o["pos"]).max(axis=(1, 2))
+        dev_c = np.abs(c["pos"] - o["pos"]).max(axis=(1, 2))
+        must = hist & hist_c
+        report[N] = dict(history_same=int(hist.sum()), control_history_same=int(hist_c.sum()), must_track=int(must.sum()),
+                         max_dev=float(dev_g[must].max()), control_max_dev=float(dev_c[must].max()))
+        assert np.all(dev_g[must] <= TRAJ_TOL), (N, report[N])
+        assert (~hist).sum() <= chaos_margin((~hist_c).sum(), 21, 21), (N, report[N])
+    print("FIRE prefix vs oracle:", report)
+    assert report[30]["must_track"] == 21 and report[100]["must_track"] >= 12
+
+
+@pytest.mark.parametrize("variant", [1, 2, 3])
+def test_fire_relaxation_config0(api, orc, variant):
+    """config 0 (benzene, 2 Morse channels) on the small slab, 48 replicas.  (a) the config as stated: 1000 FIRE steps, dt0 0.5 fs,
+    f_tol 1e-3 — with real masses few replicas converge that fast (R13), so the final states are compared;
+    (b) dt0 1 fs, dt_max 20 fs, f_tol 1e-3, 12000 steps: most replicas converge; flags and basins are compared.  Both against the chaos
+    control (module docstring, statement 2); every converged GPU state is checked as a true minimum (statement 3)."""
+    cfg = small_config(0, n_rep=48)
+    og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
+    g = gpu_grid(api, cfg["sub"], cfg["desc"])
+    ot, mol = oracle_side(orc, cfg, og), gpu_side(api, cfg)
+    vel = np.zeros_like(cfg["pos"])
+    r0 = run_gpu(api, g, mol, api.make_integrator("vv", 0, 0.5), cfg["pos"], vel)
+    e_start = r0["energy"][:, :7].astype(np.float64).sum(1)
+    Lx, Ly = cfg["desc"]["Lx"], cfg["desc"]["Ly"]
+    etot = lambda o: o["energy"][:, :7].astype(np.float64).sum(1)
+    # (a)
+    r = run_gpu(api, g, mol, api.make_integrator("fire", 1000, 0.5, f_tol=1e-3, variant=variant), cfg["pos"], vel, fire=np.zeros((48, 4), np.float32))
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 1000, 0.5, f_tol=1e-3), cfg["pos"], vel)
+    o2 = control_run(orc, og, ot, lambda n: orc.make_integrator("fire", n, 0.5, f_tol=1e-3), 1000, cfg["pos"], vel, key="c0a")
+    assert np.all(etot(r) <= e_start + 1e-6)                                   # relaxed E <= starting E
+    assert np.all(np.abs(r["energy"][:, 7]) < 1.0)
+
+    def mismatch(r, o, o2, tag):
+        (Eg, xg, cg), (Eo, xo, co), (Ec, xc, cc) = basins(orc, og, ot, r), basins(orc, og, ot, o, tag + "o"), basins(orc, og, ot, o2, tag + "c")
+        assert cg.all() and co.all() and cc.all()
+        return ~basin_match(Eg, xg, Eo, xo, Lx, Ly), ~basin_match(Ec, xc, Eo, xo, Lx, Ly), Eo
+
+    diff, diff0, Eo = mismatch(r, o, o2, "c0a")
+    print("config 0 as stated (1000 FIRE steps; converged gpu %d, oracle %d): basin mismatch gpu-vs-oracle %d/48, control (oracle with fp32 state) %d/48"
+          % ((r["status"][:, 1] == 1).sum(), (o["status"][:, 1] == 1).sum(), diff.sum(), diff0.sum()))
+    assert diff.sum() <= chaos_margin(diff0.sum(), 48, 48), (diff.sum(), diff0.sum())
+    # (b)
+    kw = dict(f_tol=1e-3, dt_max=20.0)
+    r = run_gpu(api, g, mol, api.make_integrator("fire", 12000, 1.0, variant=variant, **kw), cfg["pos"], vel, fire=np.zeros((48, 4), np.float32))
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 12000, 1.0, **kw), cfg["pos"], vel)
+    o2 = control_run(orc, og, ot, lambda n: orc.make_integrator("fire", n, 1.0, **kw), 12000, cfg["pos"], vel, key="c0b")
+    conv_g, conv_o, conv_o2 = r["status"][:, 1] == 1, o["status"][:, 1] == 1, o2["status"][:, 1] == 1
+    assert conv_o.sum() >= 20
+    assert abs(int(conv_g.sum()) - int(conv_o.sum())) <= chaos_margin(abs(int(conv_o2.sum()) - int(conv_o.sum())), 48, 48)
+    assert np.all(r["status"][conv_g, 0] < 12000)                             # a converged replica stops early
+    assert_true_minima(orc, og, ot, r["pos"][conv_g], etot(r)[conv_g], 1e-3, "config 0 (b)")
+    diff, diff0, Eo = mismatch(r, o, o2, "c0b")
+    print("config 0 relaxed (12000 steps; converged gpu %d, oracle %d, control %d): basin mismatch gpu-vs-oracle %d/48, control %d/48; %d distinct basin energies"
+          % (conv_g.sum(), conv_o.sum(), conv_o2.sum(), diff.sum(), diff0.sum(), len(np.unique(np.round(Eo, 4)))))
+    assert diff.sum() <= chaos_margin(diff0.sum(), 48, 48), (diff.sum(), diff0.sum())
+
+
+@pytest.mark.parametrize("k", [0, 2])
+def test_fire_basins_from_near_minimum_starts(api, orc, k):
+    """statement 1 (well-posed): starts = oracle minima displaced by a seeded 0.02 Å normal noise per coordinate; both sides relax with
+    f_tol = 1e-4 eV/Å; EVERY replica must converge on both sides and end in the same basin (compared after the common polish)."""
+    n_rep = 40 if k == 0 else 16
+    cfg = small_config(k, n_rep=n_rep)
+    og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
+    g = gpu_grid(api, cfg["sub"], cfg["desc"])
+    ot, mol = oracle_side(orc, cfg, og), gpu_side(api, cfg)
+    Lx, Ly = cfg["desc"]["Lx"], cfg["desc"]["Ly"]
+    E0, x0, ok = polish(orc, og, ot, cfg["pos"])
+    assert ok.sum() >= 0.75 * n_rep, ok.sum()
+    x0, E0 = x0[ok], E0[ok]
+    start = (x0 + 0.02 * np.random.default_rng(5 + k).standard_normal(x0.shape)).astype(np.float32)
+    vel = np.zeros_like(start)
+    kw = dict(f_tol=1e-4, dt_max=20.0, max_step=0.1)
+    r = run_gpu(api, g, mol, api.make_integrator("fire", 60000, 1.0, **kw), start, vel, fire=np.zeros((len(start), 4), np.float32))
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 60000, 1.0, **kw), start, vel)
+    assert np.all(r["status"][:, 1] == 1) and np.all(o["status"][:, 1] == 1), ((r["status"][:, 1] == 1).sum(), (o["status"][:, 1] == 1).sum(), len(start))
+    Eg, xg, cg = polish(orc, og, ot, r["pos"])
+    Eo, xo, co = polish(orc, og, ot, o["pos"])
+    assert cg.all() and co.all()
+    same = basin_match(Eg, xg, Eo, xo, Lx, Ly)
+    back = basin_match(Eo, xo, E0, x0, Lx, Ly)
+    print("near-minimum starts (config %d): %d/%d same basin gpu-vs-oracle; %d/%d returned to the minimum they were displaced from"
+          % (k, same.sum(), len(same), back.sum(), len(back)))
+    assert same.all(), np.nonzero(~same)[0]
+    # the GPU's own end states (before the polish) already sit in that basin and carry the oracle's energy
+    assert_true_minima(orc, og, ot, r["pos"], r["energy"][:, :7].astype(np.float64).sum(1), 1e-4, "near-minimum config %d" % k)
+
+
+def test_fire_restart_basins_config2(api, orc):
+    """config 2 on the small slab: relax -> record -> re-seed.  Minima are matched by (replica, restart#); restart conformations are the same
+    on both sides (Philox), so each pair starts from the same state.  Basins compared after the common polish, against the chaos control."""
+    cfg = small_config(2, n_rep=16)
+    og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
+    g = gpu_grid(api, cfg["sub"], cfg["desc"])
+    ot, mol = oracle_side(orc, cfg, og), gpu_side(api, cfg)
+    vel = np.zeros_like(cfg["pos"])
+    Lx, Ly = cfg["desc"]["Lx"], cfg["desc"]["Ly"]
+    # config 2's f_tol 1e-3 with dt_max 20 fs: with real masses the 60-atom chain needs 1e4-3e4 steps per minimum (R13)
+    kw = dict(f_tol=1e-3, dt_max=20.0, restart=1, seed=1002, max_step=0.1)
+    r = run_gpu(api, g, mol, api.make_integrator("fire", 40000, 1.0, **kw), cfg["pos"], vel, fire=np.zeros((16, 4), np.float32), minima_cap=2048)
+    o = orc.run_replicas(og, ot, orc.make_integrator("fire", 40000, 1.0, **kw), cfg["pos"], vel, minima_cap=2048)
+    o2 = control_run(orc, og, ot, lambda n: orc.make_integrator("fire", n, 1.0, **kw), 40000, cfg["pos"], vel, minima_cap=64)
+    assert r["n_minima"] > 0 and o["n_minima"] > 0
+    key = lambda m: {(int(x[0]), int(x[1])): x for x in m}
+    kg, ko, ko2 = key(r["minima"]), key(o["minima"]), key(o2["minima"])
+    n = cfg["pos"].shape[1]
+
+    def compare(ka, kb):
+        common = sorted(set(ka) & set(kb))
+        xa = np.array([ka[c][4:] for c in common]).reshape(len(common), n, 3); xb = np.array([kb[c][4:] for c in common]).reshape(len(common), n, 3)
+        Ea, pa, ca = polish(orc, og, ot, xa); Eb, pb, cb = polish(orc, og, ot, xb)
+        ok = ca & cb
+        return common, basin_match(Ea, pa, Eb, pb, Lx, Ly)[ok], ok
+
+    common, same, ok = compare(kg, ko)
+    common0, same0, ok0 = compare(ko2, ko)
+    print("config-2 minima: gpu %d, oracle %d, control (oracle with fp32 state) %d; common keys gpu/oracle %d (mismatch %d), control %d (mismatch %d)"
+          % (len(kg), len(ko), len(ko2), len(common), (~same).sum(), len(common0), (~same0).sum()))
+    # the two sides find minima at the same rate (a replica that converges a few steps apart records the same (replica, restart#) keys)
+    assert abs(len(kg) - len(ko)) <= chaos_margin(abs(len(ko2) - len(ko)), len(ko), len(ko)) and len(common) >= 4
+    assert (~same).sum() <= chaos_margin((~same0).sum(), len(same0), len(same)), ((~same).sum(), len(same), (~same0).sum(), len(same0))
+    # every recorded GPU minimum really is one (statement 3): stationary under the oracle's forces, the oracle's energy, stays put
+    rec = np.array([kg[c] for c in sorted(kg)][:24])
+    assert_true_minima(orc, og, ot, rec[:, 4:].reshape(len(rec), n, 3), rec[:, 3], 1e-3, "config 2 records")

@@ -59,3 +59,45 @@ def test_zero_replicas_and_too_many_atoms(api):
         api.gridff_create_molecule(big65, np.zeros((65, 4), np.float32))
     with pytest.raises(api.GridffError):
         api.gridff_run_replicas(g, mol, api.make_integrator("vv", 10, 0.5, fixed=(7,)), dev(np.zeros((2, 5, 3))), dev(np.zeros((2, 5, 3))))
+
+
+def test_many_atom_kinds_above_32_atoms(api, orc):
+    """33-64 atoms: the pair-of-warps kernel reads (R_i + R_j)^2 and 12 e_i e_j from a per-kind table when the molecule has at most 8
+    distinct Lennard-Jones kinds, and forms them per pair otherwise.  A 40-atom chain whose atoms all differ (40 kinds) takes the second
+    path; both against the oracle, and against each other on a 2-kind chain whose parameters are the same numbers."""
+    cfg = small_config(1, n_rep=1)
+    d = cfg["desc"]
+    og, _ = oracle_grid(orc, cfg["sub"], d)
+    g = gpu_grid(api, cfg["sub"], d)
+    topo = inputs.helix_chain(40, seed=9)
+    many = dict(topo)
+    many["lj_R"] = (topo["lj_R"] * (1.0 + 1e-3 * np.arange(40))).astype(np.float32)          # 40 distinct kinds
+    pos = inputs.place_replicas(topo, 11, d["Lx"], d["Ly"], 0.0, 31)
+    vel = inputs.maxwell_boltzmann(topo, 11, 300.0, 32)
+    for t in (topo, many):
+        ot = orc.OracleTopology(t, orc.atom_coefs(t["grid_e"], t["grid_R"], t["q"], d["alpha"]))
+        mol = api.gridff_create_molecule(t, api.gridff_atom_coefs(d["alpha"], t["grid_e"], t["grid_R"], t["q"]))
+        r = run_gpu(api, g, mol, api.make_integrator("vv", 40, 0.5), pos, vel)
+        o = orc.run_replicas(og, ot, orc.make_integrator("vv", 40, 0.5), pos, vel)
+        assert np.abs(r["pos"].astype(np.float64) - o["pos"]).max() <= TRAJ_TOL
+        check_energies(r["energy"], o["energy"], tol_rel=1e-4, tol_abs=2e-4)
+        r0 = run_gpu(api, g, mol, api.make_integrator("vv", 0, 0.5), pos, vel)
+        o0 = orc.run_replicas(og, ot, orc.make_integrator("vv", 0, 0.5), pos, vel)
+        check_energies(r0["energy"], o0["energy"], tol_rel=3e-5, tol_abs=3e-5)
+
+
+def test_restart_needs_the_template_conformation(api):
+    """gridff_integrator.restart = 1 re-seeds from gridff_topology.ref_pos: a molecule created without it is refused (GRIDFF_EINVAL), not run
+    from an all-zero template"""
+    cfg = small_config(1, n_rep=4)
+    d = cfg["desc"]
+    g = gpu_grid(api, cfg["sub"], d)
+    topo = dict(cfg["topo"]); topo["ref_pos"] = None; topo["rot_bond"] = None; topo["rot_mask"] = None
+    mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
+    p, v = dev(cfg["pos"]), dev(np.zeros_like(cfg["pos"]))
+    with pytest.raises(api.GridffError) as e:
+        api.gridff_run_replicas(g, mol, api.make_integrator("fire", 10, 0.5, restart=1, seed=1), p, v, d_fire=torch.zeros((4, 4), device="cuda"))
+    assert e.value.code == -1 and "ref_pos" in str(e.value)
+    out = api.gridff_run_replicas(g, mol, api.make_integrator("fire", 10, 0.5), p, v, d_fire=torch.zeros((4, 4), device="cuda"))     # without restart: fine
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(p).all()) and out["status"][:, 0].max().item() == 10

@@ -160,3 +160,28 @@ def test_coarser_grid_error_scaling(api, orc, cfg1s):
     for ch in (0, 1):
         assert 8 <= err[(0.2, ch)] / err[(0.1, ch)] <= 40, (ch, err[(0.2, ch)], err[(0.1, ch)])
     assert err[(0.1, 0)] <= 1e-4 and err[(0.1, 1)] <= 1e-5
+
+
+def test_adatom_and_z_ref_rule_of_the_coulomb_channel(api, orc):
+    """An adatom 1.1 Å above the top layer (PAPER.md:L154 defects and step edges): the Fourier sum of the Coulomb channel is cut where
+    exp(-|G| z_lo) < 1e-16, which needs every atom at least z_lo below the lowest grid plane.  z_ref below the adatom is refused
+    (GRIDFF_EINVAL); with z_ref = the adatom's z the coefficients match the oracle's to half an fp32 ulp, Coulomb channel included."""
+    sub, Lx, Ly = inputs.rocksalt_slab(2, 3, 2.82, 0.7)
+    pos = np.vstack([sub["pos"], [[1.41, 1.41, 1.1]], [[4.23, 4.23, -0.3]]])                      # +0.4 e adatom, -0.4 e interstitial: neutral
+    sub = dict(pos=pos, e=np.append(sub["e"], [0.05, 0.05]), R=np.append(sub["R"], [1.6, 1.6]), q=np.append(sub["q"], [0.4, -0.4]))
+    assert abs(sub["q"].sum()) < 1e-12
+    chans = [inputs.PAULI, inputs.LONDON, inputs.COULOMB]
+    bad = inputs.grid_desc(Lx, Ly, 0.0, 1.5, 6.5, 0.2, 1.6, chans)
+    with pytest.raises(api.GridffError) as e:
+        gpu_grid(api, sub, bad)
+    assert e.value.code == -1 and "z_ref" in str(e.value)
+    desc = inputs.grid_desc(Lx, Ly, 1.1, 1.5, 6.5, 0.2, 1.6, chans)
+    og, _ = oracle_grid(orc, sub, desc)
+    g = gpu_grid(api, sub, desc)
+    coef = api.gridff_grid_export(g).cpu().numpy().astype(np.float64)
+    for ch in range(3):
+        ref = og.coef[..., ch]
+        assert np.all(np.abs(coef[..., ch] - ref) <= 6.0e-8 * np.abs(ref) + 1e-9 * np.abs(ref).max()), ch
+    # a Morse-only grid has no such rule
+    g2 = gpu_grid(api, sub, inputs.grid_desc(Lx, Ly, 0.0, 1.5, 6.5, 0.2, 1.6, [inputs.PAULI, inputs.LONDON]))
+    assert g2.info()["n_channels"] == 2

@@ -78,3 +78,27 @@ def test_molecule_fd_and_momentum(orc, mol):
     assert E0[0] < 1e-10 and E0[1] < 1e-10
     if mol == "tetracene":
         assert E0[2] < 1e-12                                  # planar: ring torsions at their minimum
+
+
+def test_four_channel_energy_is_the_potential_of_the_forces(orc):
+    """DESIGN.md R22: with a 4-channel grid (an imported potential) the 7 reported terms sum to the potential whose gradient
+    the forces are: the fourth channel is reported with the third.  Central finite differences of sum(E7) against F, and the channel
+    split itself against per-channel interpolation."""
+    rng = np.random.default_rng(3)
+    nx = ny = 12; nz = 20; h = 0.25
+    coef = rng.normal(size=(nx, ny, nz, 4))
+    g = orc.OracleGrid(coef, nx * h, ny * h, 1.0, h)
+    n = 3
+    cf = rng.uniform(0.5, 1.5, (n, 4))
+    t = orc.OracleTopology(_topo(n), cf)
+    pos = np.array([[0.7, 1.9, 2.3], [2.2, 0.4, 3.1], [1.1, 2.6, 4.0]])
+    E7, F = orc.forces(g, t, pos)
+    _, _, Vc, _ = orc.interp(g, pos, cf, channels=True)
+    per = (cf * Vc).sum(axis=0)
+    assert np.allclose(E7[:3], [per[0], per[1], per[2] + per[3]], rtol=0, atol=1e-13) and abs(per[3]) > 1e-3
+    eps = 1e-5
+    for i in range(n):
+        for c in range(3):
+            p1, p2 = pos.copy(), pos.copy(); p1[i, c] += eps; p2[i, c] -= eps
+            dE = (orc.forces(g, t, p1)[0].sum() - orc.forces(g, t, p2)[0].sum()) / (2 * eps)
+            assert abs(dE + F[i, c]) < 1e-7 * max(1.0, abs(F[i, c]))
