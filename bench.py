@@ -522,7 +522,7 @@ def run_eval(args):
         for it in range(warm + reps):
             flush.fill_(1)
             a, b = ev(), ev()
-            a.record(stream); api.gridff_eval(g, d_pos, d_coef, d_E=d_E, d_F=d_F); b.record(stream); b.synchronize()
+            a.record(stream); api.gridff_eval(g, d_pos, d_coef, d_E=d_E, d_F=d_F, variant=args.variant or None); b.record(stream); b.synchronize()
             if it >= warm:
                 ts.append(a.elapsed_time(b))
         return ts

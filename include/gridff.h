@@ -129,7 +129,9 @@ int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const 
                 float* d_E, float* d_F, void* cuda_stream);
 
 /* Same with an explicit kernel variant (layout / gather study): 0 = library default, 1 = one thread per point
- * (64 independent 16-byte loads), 2 = warp-cooperative row gather.  A brick-layout grid always uses its own kernel. */
+ * (64 independent 16-byte loads), 2 = warp-cooperative row gather, 3 = one 3-D TMA box (cp.async.bulk.tensor, 1 KB) per point into shared
+ * memory (z-fastest fp32 stores only; GRIDFF_EUNSUPPORTED when the driver has no tensor-map entry point).  Variants 2 and 3 return
+ * bit-identical results.  A brick-layout grid always uses its own kernel. */
 int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
                         float* d_E, float* d_F, int variant, void* cuda_stream);
 

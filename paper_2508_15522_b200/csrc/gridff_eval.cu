@@ -158,6 +158,8 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
         e = launch_with_window(grid, k_eval_brick, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
     } else if (variant == 1) {
         e = launch_with_window(grid, k_eval_direct, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    } else if (variant == 3) {
+        return eval_tma(grid, n, d_pos, d_coef, d_E, d_F, st);
     } else if (variant == 0 || variant == 2) {
         const long long per_block = kEvalWarps * 32;
         e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);

@@ -1,0 +1,187 @@
+// gridff_eval_tma.cu — gridff_eval variant 3: the 4 x 4 x 4-node stencil of PAPER.md:L136 fetched as ONE 3-D TMA box per point.
+//
+// The ZFAST store (gridff_internal.cuh) is a dense tensor of 16-byte nodes with extents (nx+3) x (ny+3) x nzp; with its 3-node periodic halo
+// every stencil is an axis-aligned box {4 x, 4 y, 4 z} = 16 rows of 64 contiguous bytes = 1 KB.  That is exactly what the tensor memory
+// accelerator moves: one `cp.async.bulk.tensor.3d` (SASS UTMALDG) per point lands the box in shared memory and signals an mbarrier, without
+// occupying the LSU / L1 data pipe that bounds the warp-cooperative LDG gather (k_eval_coop: one L1 cycle per distinct 128-byte line, 22 per
+// stencil).  The tensor is described to the TMA unit as fp32 elements {nzp * 4, ny + 3, nx + 3} (z and channel merged: TMA has no
+// 16-byte element type), box {16, 4, 4}, no swizzle, no L2 promotion (a 64-byte row needs 2-3 sectors, not whole 128-byte lines).
+//
+// A warp owns 32 consecutive points and walks over its tiles persistently.  Per tile: the two halves (16 points, 16 KB each) arrive in two raw
+// buffers with their own mbarriers; the warp folds each half with the points' channel factors into the same XOR-swizzled 8 KB tile that
+// k_eval_coop builds (lanes read consecutive 16-byte chunks of the raw box: conflict-free), re-arms the half's buffer with the NEXT tile's
+// boxes, and finally every lane contracts its own point (interp_tile).  The folded tile and the contraction are bit-identical to k_eval_coop's,
+// so variant 3 returns exactly variant 2's numbers (test).  Up to 32 KB per warp and 160 KB per SM are in flight behind the arithmetic.
+#include "gridff_interp.cuh"
+#include <cuda.h>
+#include <stdio.h>
+#include <string.h>
+
+using namespace gridff;
+
+namespace {
+
+constexpr int kTmaWarps = 1;                       // warps per block: a warp is self-contained (own buffers, own barriers)
+constexpr int kRawHalf = 16 * 1024;                // 16 points x 1 KB
+constexpr size_t kWarpSmem = 2 * kRawHalf + 32 * 64 * 4 + 32 * 16 + 32 * 4 + 2 * 8;      // raw A, raw B, folded tile, cf, base, 2 mbarriers
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// one {16 floats, 4, 4} box: fastest coordinate first (z * 4 + channel, y, x), in elements
+__device__ __forceinline__ void tma_box(void* dst, const CUtensorMap* map, int c0, int c1, int c2, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
+
+struct Pt { unsigned base; float tx, ty, tz; int c0, c1, c2; float4 cf; };
+
+__device__ __forceinline__ Pt load_point(const GridGeom& g, long long p, long long n, const float* __restrict__ pos, const float4* __restrict__ coef) {
+    Pt q; q.base = kNoStencil; q.tx = q.ty = q.tz = 0.f; q.c0 = q.c1 = q.c2 = 0; q.cf = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (p < n) {
+        int ix, iy, iz;
+        cell_periodic(pos[3 * p], g.inv_hx_hi, g.inv_hx_lo, g.fnx, g.inv_nx, ix, q.tx);
+        cell_periodic(pos[3 * p + 1], g.inv_hy_hi, g.inv_hy_lo, g.fny, g.inv_ny, iy, q.ty);
+        if (cell_z(pos[3 * p + 2], g, iz, q.tz)) {
+            q.base = (unsigned)corner_zfast(g, ix, iy, iz);        // same validity flag and offsets as the LDG kernels
+            q.c0 = 4 * (iz - 1); q.c1 = iy; q.c2 = ix;             // stored index s holds node s - 1: the stencil corner (ix-1, iy-1) is stored at (ix, iy)
+        } else q.tz = 0.f;
+        q.cf = coef[p];
+    }
+    return q;
+}
+
+__global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_constant__ CUtensorMap tmap, GridGeom g, long long n, const float* __restrict__ pos,
+                                                             const float4* __restrict__ coef, float* __restrict__ E, float* __restrict__ F) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned char* base = smem + ((128u - (smem_u32(smem) & 127u)) & 127u) + (size_t)w * ((kWarpSmem + 1023) & ~(size_t)1023);    // TMA destinations: 128-byte aligned
+    float4* raw[2] = {reinterpret_cast<float4*>(base), reinterpret_cast<float4*>(base + kRawHalf)};
+    float* tile = reinterpret_cast<float*>(base + 2 * kRawHalf);
+    float4* s_cf = reinterpret_cast<float4*>(tile + 32 * 64);
+    unsigned* s_base = reinterpret_cast<unsigned*>(s_cf + 32);
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_base + 32);
+    if (lane == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+
+    const long long n_tiles = (n + 31) / 32, stride = (long long)gridDim.x * kTmaWarps;
+    long long t = (long long)blockIdx.x * kTmaWarps + w;
+    const int half = lane >> 4;
+    // arm one half-buffer with the boxes of the points of `q` that sit in it (the lanes of that half own them)
+    auto issue = [&](const Pt& q, int hb) {
+        const unsigned valid = __ballot_sync(0xFFFFFFFFu, q.base != kNoStencil);
+        const unsigned mine = (valid >> (16 * hb)) & 0xFFFFu;
+        if (lane == 0) mbar_expect_tx(bar + hb, 1024u * (unsigned)__popc(mine));
+        __syncwarp();
+        if (half == hb && q.base != kNoStencil) tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
+    };
+    Pt cur = load_point(g, t * 32 + lane, n, pos, coef);
+    if (t < n_tiles) { issue(cur, 0); issue(cur, 1); }
+    unsigned parity = 0;
+    for (; t < n_tiles; t += stride) {
+        const long long tn = t + stride;
+        Pt nxt = load_point(g, tn < n_tiles ? tn * 32 + lane : n, n, pos, coef);       // p = n: an empty point
+        s_cf[lane] = cur.cf; s_base[lane] = cur.base;
+        __syncwarp();
+#pragma unroll
+        for (int hb = 0; hb < 2; ++hb) {
+            mbar_wait(bar + hb, parity);
+            const float4* r4 = raw[hb];
+#pragma unroll 4
+            for (int q = 0; q < 16; ++q) {
+                if (s_base[16 * hb + q] != kNoStencil)
+                    store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], lane, 16 * hb + q, tile);
+            }
+            __syncwarp();                                  // every lane has read this half: the buffer can take the next tile's boxes
+            if (tn < n_tiles) issue(nxt, hb);
+        }
+        parity ^= 1;
+        __syncwarp();
+        const long long p = t * 32 + lane;
+        if (p < n) {
+            Stencil s; s.base = cur.base; s.tx = cur.tx; s.ty = cur.ty; s.tz = cur.tz;
+            float e, fx, fy, fz;
+            interp_tile(g, s, lane, tile, e, fx, fy, fz);
+            if (E) E[p] = e;
+            if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
+        }
+        __syncwarp();                                      // the folded tile and s_cf / s_base are rewritten in the next trip
+        cur = nxt;
+    }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+}  // namespace
+
+namespace gridff {
+
+// Encode the ZFAST store as a 3-D tensor of fp32 {nzp * 4, sy, sx} with a {16, 4, 4} box (driver entry point looked up at run time: the
+// library does not link libcuda).  Returns 0 and fills grid->tmap on success.
+int make_tensor_map(gridff_grid* grid) {
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr; cudaDriverEntryPointQueryResult qr;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr);
+        if (e != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) { cudaGetLastError(); set_error("cuTensorMapEncodeTiled is not available in this driver"); return GRIDFF_EUNSUPPORTED; }
+        encode = (EncodeTiledFn)fn;
+    }
+    const GridGeom& G = grid->geom;
+    static_assert(sizeof(CUtensorMap) <= sizeof(grid->tmap), "tensor map storage");
+    const cuuint64_t dims[3] = {(cuuint64_t)G.nzp * 4, (cuuint64_t)G.sy, (cuuint64_t)G.sx};
+    const cuuint64_t strides[2] = {(cuuint64_t)G.nzp * 16, (cuuint64_t)G.sy * G.nzp * 16};         // bytes, dims 1 and 2
+    const cuuint32_t box[3] = {16, 4, 4}, estr[3] = {1, 1, 1};
+    CUtensorMap m;
+    CUresult r = encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)G.store, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (%d)", (int)r); return GRIDFF_ECUDA; }
+    memcpy(grid->tmap, &m, sizeof(m));
+    grid->tmap_ok = 1;
+    return GRIDFF_OK;
+}
+
+int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st) {
+    if (!grid->tmap_ok) { set_error("this grid has no tensor map (TMA needs the z-fastest fp32 store)"); return GRIDFF_EUNSUPPORTED; }
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const size_t smem = kTmaWarps * ((kWarpSmem + 1023) & ~(size_t)1023) + 128;
+    static bool attr_set = false;
+    if (!attr_set) {
+        GRIDFF_CUDA(cudaFuncSetAttribute(k_eval_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GRIDFF_CUDA(cudaFuncSetAttribute(k_eval_tma, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        attr_set = true;
+    }
+    int per_sm = 1;
+    GRIDFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_eval_tma, kTmaWarps * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+    const long long n_tiles = (n + 31) / 32;
+    long long blocks = (long long)sms * per_sm;
+    if (blocks * kTmaWarps > n_tiles) blocks = (n_tiles + kTmaWarps - 1) / kTmaWarps;
+    CUtensorMap m;
+    memcpy(&m, grid->tmap, sizeof(m));
+    cudaError_t e = launch_with_window(grid, k_eval_tma, dim3((unsigned)blocks), dim3(kTmaWarps * 32), smem, st, m, grid->geom, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    count_launch();
+    if (e != cudaSuccess) return cuda_fail(e, "gridff_eval (TMA) launch");
+    return GRIDFF_OK;
+}
+
+}  // namespace gridff

@@ -35,6 +35,8 @@ int molecule_n_atoms(const gridff_molecule* mol);     // gridff_replica.cu (the 
 
 void set_error(const char* fmt, ...);
 int eval_derived(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);   // gridff_derive.cu
+int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);       // gridff_eval_tma.cu
+int make_tensor_map(gridff_grid* grid);               // gridff_eval_tma.cu: CUtensorMap of a z-fastest fp32 store (0 on success)
 int cuda_fail(cudaError_t e, const char* what);
 void count_launch(int n = 1);
 
@@ -111,4 +113,6 @@ struct gridff_grid {
     double h[3], origin[3];
     size_t store_bytes;
     int l2_window_ok;     // 1 when an access-policy window could be applied
+    int tmap_ok;          // 1 when tmap describes the store (z-fastest fp32 stores; gridff_eval variant 3)
+    alignas(64) unsigned char tmap[128];      // CUtensorMap (opaque here: <cuda.h> is needed only where it is encoded and used)
 };

@@ -132,8 +132,8 @@ def test_config3_full_size_oracle_parity(api, orc):
         for i0 in range(0, 400, 50):                              # in slabs: the fp64 difference of the whole array would be another 190 MB
             err = np.abs(got[i0:i0 + 50].astype(np.float64) - ref[i0:i0 + 50])
             assert np.all(err <= 6.0e-8 * np.abs(ref[i0:i0 + 50]) + 1e-9 * scale), (c, i0, err.max(), scale)
-            worst = max(worst, float((err / (np.abs(ref[i0:i0 + 50]) + 1e-9 * scale)).max()))
-        print("channel %d: all 24 M coefficients within %.2e relative of the oracle's" % (c, worst))
+            worst = max(worst, float((err / (6.0e-8 * np.abs(ref[i0:i0 + 50]) + 1e-9 * scale)).max()))
+        print("channel %d: all 24 M coefficients within the tolerance (half an fp32 ulp + 1e-9 of the channel's scale); worst uses %.2f of it" % (c, worst))
     del coef, got
     # (2)
     z0 = d["z_ref"] + d["z_lo"]

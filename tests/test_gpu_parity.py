@@ -95,7 +95,7 @@ def eval_points(cfg, n, seed, rng_z=(1.55, 8.6)):
     return pos, coef
 
 
-@pytest.mark.parametrize("k,variant,layout", [(1, 1, 0), (1, 2, 0), (1, 0, 1), (3, 1, 0), (3, 2, 0)])
+@pytest.mark.parametrize("k,variant,layout", [(1, 1, 0), (1, 2, 0), (1, 3, 0), (1, 0, 1), (3, 1, 0), (3, 2, 0), (3, 3, 0)])
 def test_eval_parity(api, orc, cfg1s, cfg3s, k, variant, layout):
     cfg = cfg1s if k == 1 else cfg3s
     og, _ = oracle_grid(orc, cfg["sub"], cfg["desc"])
@@ -113,6 +113,21 @@ def test_eval_parity(api, orc, cfg1s, cfg3s, k, variant, layout):
     ok = den > 1e-12
     assert rel[ok].max() <= E_REL_TOL, rel[ok].max()
     assert np.abs(Fg - Fo).max() <= F_ABS_TOL, np.abs(Fg - Fo).max()
+
+
+def test_eval_tma_variant_is_bit_identical(api, cfg1s):
+    """variant 3 (one 3-D TMA box per point, folded into the same swizzled tile) returns exactly variant 2's numbers (the warp-cooperative
+    LDG gather), whatever the point count (persistent warps: 1 point, less than a tile, many tiles per warp) and with E or F alone"""
+    g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
+    for n in (1, 31, 33, 5000, 300007):
+        pos, coef = eval_points(cfg1s, n, 100 + n)
+        dp, dc = dev(pos), dev(coef)
+        E2, F2 = api.gridff_eval(g, dp, dc, variant=2)
+        E3, F3 = api.gridff_eval(g, dp, dc, variant=3)
+        assert bool(torch.equal(E2, E3)) and bool(torch.equal(F2, F3)), n
+    E3, none = api.gridff_eval(g, dp, dc, variant=3, want_F=False)
+    none2, F3b = api.gridff_eval(g, dp, dc, variant=3, want_E=False)
+    assert none is None and none2 is None and bool(torch.equal(E3, E2)) and bool(torch.equal(F3b, F2))
 
 
 def test_eval_edge_cases(api, cfg1s):
