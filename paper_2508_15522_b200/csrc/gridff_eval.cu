@@ -1,6 +1,7 @@
 // gridff_eval.cu — gridff_eval (step a5) and the bandwidth probe.  PAPER.md:L128-138; DESIGN.md §5.
 #include "gridff_interp.cuh"
 #include <stdio.h>
+#include <atomic>
 
 using namespace gridff;
 
@@ -23,8 +24,10 @@ __global__ void __launch_bounds__(128) k_eval_direct(GridGeom g, long long n, co
 // its own point from the (swizzled) tile.
 constexpr int kEvalWarps = 4;
 
+// `choice` (may be NULL): device word written by k_eval_classify; the kernel runs only when it holds kChoiceCoop
 __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
-                                                               float* __restrict__ E, float* __restrict__ F) {
+                                                               float* __restrict__ E, float* __restrict__ F, const unsigned* __restrict__ choice) {
+    if (choice && *choice != kChoiceCoop) return;
     __shared__ __align__(16) float s_tile[kEvalWarps][32 * 64];
     __shared__ __align__(16) float4 s_cf[kEvalWarps][32];
     __shared__ unsigned s_base[kEvalWarps][32];
@@ -32,14 +35,13 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
     const long long p = ((long long)blockIdx.x * kEvalWarps + w) * 32 + lane;
     Stencil s; s.base = kNoStencil; s.tx = s.ty = s.tz = 0.f;
     float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2]); cf = coef[p]; }
+    int ix = 0, iy = 0, iz = 0;
+    if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz); cf = coef[p]; }
     s_base[w][lane] = s.base; s_cf[w][lane] = cf;
     __syncwarp();
     float* tile = s_tile[w];
-    // do this warp's points share stencils?  (spatially sorted input: most lanes sit in their neighbour's cell)  Then the L1 pays;
-    // otherwise gather past it
-    const unsigned prev = __shfl_up_sync(0xFFFFFFFFu, s.base, 1);
-    const bool clustered = __popc(__ballot_sync(0xFFFFFFFFu, lane > 0 && prev == s.base)) >= 8;
+    // do this warp's points share stencil lines?  (spatially sorted input)  Then the L1 pays; otherwise gather past it
+    const bool clustered = warp_points_are_local(ix, iy, iz, s.base != kNoStencil, lane);
     if (clustered) {
 #pragma unroll 8
         for (int q = 0; q < 32; ++q) {
@@ -60,6 +62,33 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
     if (E) E[p] = e;
     if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
 }
+
+// Which kernel for a store that does not fit the L2?  Scattered points: the TMA box kernel (DRAM-bound, it keeps more bytes in flight: +26 %);
+// spatially sorted points: the LDG gather at full occupancy (L2 hits: 2.3x).  The order of the caller's points is not known at launch, so a
+// one-block kernel samples 64 warp tiles spread over the array, applies warp_points_are_local and leaves the choice in a device word that both
+// kernels read first; the one not chosen exits at once.  No host round-trip.
+__global__ void __launch_bounds__(256) k_eval_classify(GridGeom g, long long n, const float* __restrict__ pos, unsigned* __restrict__ choice) {
+    __shared__ int s_local[8];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const long long n_tiles = (n + 31) / 32;
+    int local = 0;
+    for (int k = 0; k < 8; ++k) {
+        const long long t = (long long)((double)(8 * w + k) * (double)n_tiles / 64.0);
+        const long long p = t * 32 + lane;
+        int ix = 0, iy = 0, iz = 0; bool valid = false;
+        if (p < n) valid = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz).base != kNoStencil;
+        local += warp_points_are_local(ix, iy, iz, valid, lane) ? 1 : 0;
+    }
+    if (lane == 0) s_local[w] = local;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+        for (int k = 0; k < 8; ++k) tot += s_local[k];
+        *choice = tot >= 32 ? kChoiceCoop : kChoiceTma;
+    }
+}
+
+__device__ unsigned g_eval_choice[64];        // one word per launch in flight (round robin): concurrent streams do not share a word
 
 // brick layout, thread per point (layout study)
 __device__ __forceinline__ size_t brick_index(const GridGeom& g, int s_x, int s_y, int iz) {
@@ -138,6 +167,16 @@ __global__ void __launch_bounds__(256) k_probe_rows(const float4* __restrict__ b
     if (acc == 1.2345678e-30f) *sink = acc;
 }
 
+bool store_exceeds_l2(const gridff_grid* grid) {
+    static int l2_bytes = -1;
+    if (l2_bytes < 0) {
+        int dev = 0, v = 0;
+        cudaGetDevice(&dev);
+        l2_bytes = cudaDeviceGetAttribute(&v, cudaDevAttrL2CacheSize, dev) == cudaSuccess ? v : 0;
+    }
+    return l2_bytes > 0 && grid->store_bytes > (size_t)l2_bytes;
+}
+
 }  // namespace
 
 
@@ -159,10 +198,24 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
     } else if (variant == 1) {
         e = launch_with_window(grid, k_eval_direct, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
     } else if (variant == 3) {
-        return eval_tma(grid, n, d_pos, d_coef, d_E, d_F, st);
+        return eval_tma(grid, n, d_pos, d_coef, d_E, d_F, nullptr, st);
     } else if (variant == 0 || variant == 2) {
+        // default for a store that does not fit the L2: classify the point order on the device, then launch both kernels (see k_eval_classify).
+        // L2-resident stores: the LDG gather alone (1.4x the TMA kernel there).
+        unsigned* choice = nullptr;
+        if (variant == 0 && grid->tmap_ok && n >= 4096 && store_exceeds_l2(grid)) {
+            static std::atomic<unsigned> next{0};
+            unsigned* words = nullptr;
+            GRIDFF_CUDA(cudaGetSymbolAddress((void**)&words, g_eval_choice));
+            choice = words + (next.fetch_add(1, std::memory_order_relaxed) & 63u);
+            k_eval_classify<<<1, 256, 0, st>>>(G, n, d_pos, choice);
+            GRIDFF_LAUNCH_CHECK("k_eval_classify");
+            int rc = eval_tma(grid, n, d_pos, d_coef, d_E, d_F, choice, st);
+            if (rc) return rc;
+        }
         const long long per_block = kEvalWarps * 32;
-        e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+        e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F,
+                               (const unsigned*)choice);
     } else { set_error("unknown eval variant %d", variant); return GRIDFF_EINVAL; }
     count_launch();
     if (e != cudaSuccess) return cuda_fail(e, "gridff_eval launch");

@@ -68,7 +68,9 @@ __device__ __forceinline__ Pt load_point(const GridGeom& g, long long p, long lo
 }
 
 __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_constant__ CUtensorMap tmap, GridGeom g, long long n, const float* __restrict__ pos,
-                                                             const float4* __restrict__ coef, float* __restrict__ E, float* __restrict__ F) {
+                                                             const float4* __restrict__ coef, float* __restrict__ E, float* __restrict__ F,
+                                                             const unsigned* __restrict__ choice) {
+    if (choice && *choice != kChoiceTma) return;          // gridff_eval's device-side choice (k_eval_classify) went to the LDG kernel
     extern __shared__ __align__(16) unsigned char smem[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     unsigned char* base = smem + ((128u - (smem_u32(smem) & 127u)) & 127u) + (size_t)w * ((kWarpSmem + 1023) & ~(size_t)1023);    // TMA destinations: 128-byte aligned
@@ -92,27 +94,41 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
         __syncwarp();
         if (half == hb && q.base != kNoStencil) tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
     };
+    // A tile whose points share stencil lines (spatially sorted input: warp_points_are_local) is gathered through the L1 instead, as k_eval_coop
+    // does: L1 / L2 hits are worth more than the TMA's independence from the LSU.  Its buffers are simply not armed.
+    auto is_clustered = [&](const Pt& q) { return warp_points_are_local(q.c2, q.c1, q.c0 >> 2, q.base != kNoStencil, lane); };
     Pt cur = load_point(g, t * 32 + lane, n, pos, coef);
-    if (t < n_tiles) { issue(cur, 0); issue(cur, 1); }
+    bool cur_cl = is_clustered(cur);
+    if (t < n_tiles && !cur_cl) { issue(cur, 0); issue(cur, 1); }
     unsigned parity = 0;
     for (; t < n_tiles; t += stride) {
         const long long tn = t + stride;
         Pt nxt = load_point(g, tn < n_tiles ? tn * 32 + lane : n, n, pos, coef);       // p = n: an empty point
+        const bool nxt_cl = is_clustered(nxt);
         s_cf[lane] = cur.cf; s_base[lane] = cur.base;
         __syncwarp();
-#pragma unroll
-        for (int hb = 0; hb < 2; ++hb) {
-            mbar_wait(bar + hb, parity);
-            const float4* r4 = raw[hb];
-#pragma unroll 4
-            for (int q = 0; q < 16; ++q) {
-                if (s_base[16 * hb + q] != kNoStencil)
-                    store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], lane, 16 * hb + q, tile);
+        if (cur_cl) {
+#pragma unroll 8
+            for (int q = 0; q < 32; ++q) {
+                const unsigned b = s_base[q];
+                if (b != kNoStencil) gather_rows<false>(g, b, s_cf[q], lane, q, tile);
             }
-            __syncwarp();                                  // every lane has read this half: the buffer can take the next tile's boxes
-            if (tn < n_tiles) issue(nxt, hb);
+            if (tn < n_tiles && !nxt_cl) { issue(nxt, 0); issue(nxt, 1); }
+        } else {
+#pragma unroll
+            for (int hb = 0; hb < 2; ++hb) {
+                mbar_wait(bar + hb, parity);
+                const float4* r4 = raw[hb];
+#pragma unroll 4
+                for (int q = 0; q < 16; ++q) {
+                    if (s_base[16 * hb + q] != kNoStencil)
+                        store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], lane, 16 * hb + q, tile);
+                }
+                __syncwarp();                              // every lane has read this half: the buffer can take the next tile's boxes
+                if (tn < n_tiles && !nxt_cl) issue(nxt, hb);
+            }
+            parity ^= 1;
         }
-        parity ^= 1;
         __syncwarp();
         const long long p = t * 32 + lane;
         if (p < n) {
@@ -123,7 +139,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
             if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
         }
         __syncwarp();                                      // the folded tile and s_cf / s_base are rewritten in the next trip
-        cur = nxt;
+        cur = nxt; cur_cl = nxt_cl;
     }
 }
 
@@ -150,15 +166,18 @@ int make_tensor_map(gridff_grid* grid) {
     const cuuint64_t strides[2] = {(cuuint64_t)G.nzp * 16, (cuuint64_t)G.sy * G.nzp * 16};         // bytes, dims 1 and 2
     const cuuint32_t box[3] = {16, 4, 4}, estr[3] = {1, 1, 1};
     CUtensorMap m;
+    // L2 promotion: measured on the 1.09 GB store, random points: NONE 2.20e9, 64 B 2.30e9, 128 B 2.20e9, 256 B 1.96e9 evals/s (every setting
+    // moves whole 128-byte lines from DRAM: 2.6 KB per point, profiles/r2_hbm.md)
+    const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_L2_64B;
     CUresult r = encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)G.store, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                        CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                        CU_TENSOR_MAP_SWIZZLE_NONE, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (%d)", (int)r); return GRIDFF_ECUDA; }
     memcpy(grid->tmap, &m, sizeof(m));
     grid->tmap_ok = 1;
     return GRIDFF_OK;
 }
 
-int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st) {
+int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, const unsigned* d_choice, cudaStream_t st) {
     if (!grid->tmap_ok) { set_error("this grid has no tensor map (TMA needs the z-fastest fp32 store)"); return GRIDFF_EUNSUPPORTED; }
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
@@ -178,7 +197,7 @@ int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const flo
     if (blocks * kTmaWarps > n_tiles) blocks = (n_tiles + kTmaWarps - 1) / kTmaWarps;
     CUtensorMap m;
     memcpy(&m, grid->tmap, sizeof(m));
-    cudaError_t e = launch_with_window(grid, k_eval_tma, dim3((unsigned)blocks), dim3(kTmaWarps * 32), smem, st, m, grid->geom, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    cudaError_t e = launch_with_window(grid, k_eval_tma, dim3((unsigned)blocks), dim3(kTmaWarps * 32), smem, st, m, grid->geom, n, d_pos, (const float4*)d_coef, d_E, d_F, d_choice);
     count_launch();
     if (e != cudaSuccess) return cuda_fail(e, "gridff_eval (TMA) launch");
     return GRIDFF_OK;

@@ -35,7 +35,8 @@ int molecule_n_atoms(const gridff_molecule* mol);     // gridff_replica.cu (the 
 
 void set_error(const char* fmt, ...);
 int eval_derived(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);   // gridff_derive.cu
-int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);       // gridff_eval_tma.cu
+constexpr unsigned kChoiceCoop = 1u, kChoiceTma = 2u;     // device-side kernel choice of gridff_eval (gridff_eval.cu: k_eval_classify)
+int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, const unsigned* d_choice, cudaStream_t st);       // gridff_eval_tma.cu
 int make_tensor_map(gridff_grid* grid);               // gridff_eval_tma.cu: CUtensorMap of a z-fastest fp32 store (0 on success)
 int cuda_fail(cudaError_t e, const char* what);
 void count_launch(int n = 1);

@@ -13,13 +13,28 @@ struct Stencil {           // where an atom sits in the grid
 };
 constexpr unsigned kNoStencil = 0xFFFFFFFFu;
 
-__device__ __forceinline__ Stencil locate(const GridGeom& g, float x, float y, float z) {
-    Stencil s; int ix, iy, iz;
+__device__ __forceinline__ Stencil locate(const GridGeom& g, float x, float y, float z, int& ix, int& iy, int& iz) {
+    Stencil s;
     cell_periodic(x, g.inv_hx_hi, g.inv_hx_lo, g.fnx, g.inv_nx, ix, s.tx);
     cell_periodic(y, g.inv_hy_hi, g.inv_hy_lo, g.fny, g.inv_ny, iy, s.ty);
     if (cell_z(z, g, iz, s.tz)) s.base = (unsigned)corner_zfast(g, ix, iy, iz);
-    else { s.base = kNoStencil; s.tz = 0.f; }
+    else { s.base = kNoStencil; s.tz = 0.f; iz = 0; }
     return s;
+}
+__device__ __forceinline__ Stencil locate(const GridGeom& g, float x, float y, float z) {
+    int ix, iy, iz;
+    return locate(g, x, y, z, ix, iy, iz);
+}
+
+// Do the 32 points of a warp share stencil lines?  True when at least 12 lanes sit within 3 cells in x and y and 7 in z of the point of the
+// lane before them (spatially sorted input, dense or sparse); then gathering through the L1 pays.  ix, iy, iz: the lane's
+// cell, valid: the lane has a stencil.
+__device__ __forceinline__ bool warp_points_are_local(int ix, int iy, int iz, bool valid, int lane) {
+    const unsigned full = 0xFFFFFFFFu;
+    const int px = __shfl_up_sync(full, ix, 1), py = __shfl_up_sync(full, iy, 1), pz = __shfl_up_sync(full, iz, 1);
+    const bool pv = __shfl_up_sync(full, (int)valid, 1) != 0;
+    const bool near = lane > 0 && valid && pv && abs(ix - px) <= 3 && abs(iy - py) <= 3 && abs(iz - pz) <= 7;
+    return __popc(__ballot_sync(full, near)) >= 12;
 }
 
 __device__ __forceinline__ float fold4(const float4 c, const float4 n) {
