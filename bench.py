@@ -43,6 +43,7 @@ def parse():
     ap.add_argument("--replicas", type=int, default=0, help="override the config's replica count (0 = config value)")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-also", action="store_true", help="default (config 1, N = 1) run: skip the short extra measurements of configs 2, 3 and 4 reported under 'also'")
     ap.add_argument("--mode", default="run", choices=["run", "langevin", "hopping", "scan"],
                     help="SURVEY §8(f) rows on the chosen replica config: langevin = kind 2 instead of the config's integrator; hopping = "
                          "gridff_minima_hopping cycles (1000 Langevin steps at 300 K + FIRE); scan = gridff_run_scan lift of one held atom")
@@ -60,7 +61,8 @@ def workload(args):
     md = args.md_steps or cfg["integ"]["n_steps"]
     nx, ny, nz = inputs.grid_dims(cfg["desc"])
     name = {0: "config0: NaCl(001) 4x4 slab, 2 channels, 64 x benzene, FIRE x 1000",
-            2: "config2: config1 grid, 16384 x 60-atom flexible chain, FIRE to 1e-3 eV/A (cap 20000) + Philox restart",
+            2: "config2: config1 grid, 16384 x 60-atom flexible chain, FIRE (dt0 0.5 fs, dt_max 20 fs, displacement cap 0.1 A per step) to 1e-3 eV/A, "
+               "cap 20000 iterations per launch, + Philox restart; batches above 256 replicas start from 256 seeded conformers",
             1: "config1: NaCl(001) 4x4 slab + Coulomb, 4096 x 30-atom aromatic, VV dt 0.5 fs x 10000",
             3: "config3: 40x40 Å slab, 400x400x150x4 grid (384 MB), 8192 x 30-atom aromatic, VV x 5000"}[args.config]
     return cfg, md, (nx, ny, nz), name
@@ -105,24 +107,35 @@ def run_reference(args):
         return
     cfg, md, dims, name = workload(args)
     total = cfg["n_rep"] * md
-    times = []
+    times, extrap = [], []
     for it in range(args.warmup + args.steps):
         tb, tps, cores, n, ss = oracle_sample(cfg, md)
         if it >= args.warmup:
-            times.append(tb + total * tps)           # whole-workload time extrapolated from the sample
+            times.append(tb + n * ss * tps)          # MEASURED: one step of the sample = grid build + n replicas x ss steps
+            extrap.append(total / (tb + total * tps))
     t = float(np.mean(times))
-    val = total / t
-    sample = "full grid build (a1-a3) + %d replicas x %d steps, extrapolated to %d x %d" % (n, ss, cfg["n_rep"], md)
+    val = n * ss / t                                 # replica-steps/s of the sample as run (nothing projected)
+    sample = ("one step = the whole fp64 grid build (a1-a3) + %d replicas x %d steps (a5-a9) of the %d x %d workload; value = those replica-steps / the "
+              "measured time; 'extrapolated_full_workload' = the same two measured rates projected to the whole workload" % (n, ss, cfg["n_rep"], md))
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": name, "grid": list(dims), "n_replicas": cfg["n_rep"], "md_steps_per_step": md, "atoms": int(cfg["topo"]["n_atoms"])},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample, "extrapolated_full_workload": float(np.mean(extrap))},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
 
 
 # ------------------------------------------------------------------------------------------------------------------ GPU arm
+
+def ncu_facts(key):
+    """what ncu measured for this config's dominant kernel at the last capture (profiles/ncu_facts.json, written from the committed
+    captures): measured L2 -> L1 bytes, pipe utilisations, the binding unit.  None when no capture exists for the config."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "ncu_facts.json"))).get(key)
+    except Exception:
+        return None
+
 
 class ClockSampler:
     Q = "index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
@@ -214,7 +227,8 @@ def run_f_rows(args):
                       "gpu_launches": int(api.gridff_launch_count() - l0), "details": extra}))
 
 
-def run_gridff(args):
+def run_gridff(args, emit=True):
+    """one JSON line for a replica config (emit) or the same dict returned (the 'also' entries of the default run)"""
     import torch
     import torch.distributed as dist
     from paper_2508_15522_b200 import api, shard     # api raises if the CUDA library is missing: there is no fallback
@@ -222,7 +236,7 @@ def run_gridff(args):
     world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
-    if world > 1:
+    if world > 1 and not dist.is_initialized():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     cfg, md, dims, name = workload(args)
@@ -378,30 +392,72 @@ def run_gridff(args):
                 "peak_source": ("L2 read bandwidth measured in this run by gridff_probe_read (coalesced 16 B loads over a %d MB buffer)" % (probe.numel() >> 20))
                 if store_fits_l2 else hbm_src,
                 "l2_probe_gbs": l2, "hbm_peak_gbs": hbm_peak, "frac_of_hbm_peak": achieved / hbm_peak,
+                "achieved_is": "ALGORITHMIC gather bytes (64 nodes x 16 B per atom-grid evaluation) / kernel time — north_star's gather roofline, not a "
+                               "measured L2 transfer rate: the kernel keeps each atom's folded stencil in shared memory and re-gathers it only when the atom "
+                               "changes cell, so the bytes that really cross L2 -> L1 are a small fraction ('ncu' below)",
                 "bound_definition": "north_star's gather roofline: algorithmic stencil bytes over the measured L2 read bandwidth when the store fits "
                                     "the L2 ('l2'), over the measured HBM bandwidth otherwise ('hbm'); frac_of_hbm_peak is always given as well",
-                "binding_unit": "ncu (profiles/r1c_profiles.md): shared-memory data pipe 85 %, issue slots 70 %; L2->L1 traffic 2 TB/s"}
+                "ncu": ncu_facts("config%d" % args.config)}
 
     cpu = None
     if not args.no_cpu_baseline:
         tb, tps, cores, n, ss = oracle_sample(cfg, md)
         tot = units
-        cpu = {"value": tot / (tb + tot * tps), "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "full fp64 grid build (a1-a3, %.1f s) + %d replicas x %d steps (%.3g s per replica-step), extrapolated to %d x %d" % (tb, n, ss, tps, n_rep, md),
-               "replica_steps_per_s_run_only": 1.0 / tps}
+        cpu = {"value": n * ss / (tb + n * ss * tps), "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "MEASURED on the sample: the whole fp64 grid build (a1-a3, %.1f s) + %d replicas x %d steps (a5-a9, %.3g s per replica-step) of the "
+                         "%d x %d workload; value = those replica-steps / that time" % (tb, n, ss, tps, n_rep, md),
+               "extrapolated_full_workload": tot / (tb + tot * tps), "replica_steps_per_s_run_only": 1.0 / tps}
 
-    print(json.dumps({
+    line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": name, "grid": list(dims), "channels": len(d["channels"]), "store_bytes": sb, "n_replicas_per_gpu": n_rep,
                    "md_steps_per_step": md, "atoms": n_at, "integrator": kind, "variant": args.variant, "parallelism": "replicas only (no collective)",
                    "l2_flush_between_steps": True, "step": "gridff_build_grid + gridff_run_replicas"},
-        "atom_grid_evals_per_s": value * n_at, "sampling": sampling,
+        "atom_grid_evals_per_s": value * n_at, "kernel_only_replica_steps_per_s": units / (kern_ms * 1e-3), "sampling": sampling,
         "ms_build_grid": ms_per_step - kern_ms,
         "clocks": clocks, "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}))
+        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu}
+    if not emit:
+        return line
+    if world == 1 and args.config == 1 and not args.no_also and not args.md_steps and not args.replicas:
+        torch.cuda.empty_cache()
+        line["also"] = also_entries(args)
+    print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def also_entries(args):
+    """The second half of BASELINE.json's metric ("atom-grid evals/s AND replica MD steps/s") and the other replica configs, measured briefly
+    (2 timed steps after 3 warm-ups each, device-timed, L2 flushed) after the main timed region of the default run, so that the driver's record
+    of `python bench.py` carries them: config 2 (60-atom FIRE + restart), config 3 (384 MB grid), config 4 on the config-1 grid and on the
+    512 x 512 x 256 sweep grid (1.09 GB: the HBM-bound gather), random and Morton-sorted points."""
+    import argparse
+    out = {}
+    base = dict(vars(args), steps=2, warmup=3, no_cpu_baseline=True, no_also=True, md_steps=0, replicas=0, variant=0, mode="run")
+    todo = [("config2", dict(config=2)), ("config3", dict(config=3)),
+            ("config4_random", dict(config=4, order="random", c4_grid="config1", log2_points=26)),
+            ("config4_sorted", dict(config=4, order="sorted", c4_grid="config1", log2_points=26)),
+            ("config4_hbm_512x512x256_random", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25)),
+            ("config4_hbm_512x512x256_sorted", dict(config=4, order="sorted", c4_grid="512x512x256", log2_points=25))]
+    for key, kw in todo:
+        a = argparse.Namespace(**dict(base, c4_store="fp32", sweep=False, **kw))
+        t0 = time.perf_counter()
+        try:
+            r = run_eval(a, emit=False) if a.config == 4 else run_gridff(a, emit=False)
+            rf = r["roofline"]
+            out[key] = {"metric": r["metric"], "value": r["value"], "unit": r["unit"], "ms_per_step": r["ms_per_step"], "kernel_ms": rf["kernel_ms"],
+                        "roofline": {k: rf[k] for k in ("bound", "achieved", "peak", "unit", "frac", "traffic")}, "e2e": r["e2e"],
+                        "workload": r["config"]["workload"], "gpu_launches": r["gpu_launches"], "wall_s": None}
+            if r.get("sampling"):
+                out[key]["relaxed_configs_per_s"] = r["sampling"]["relaxed_configs_per_s"]
+            if "ms_build_grid" in r:
+                out[key]["ms_build_grid"] = r["ms_build_grid"]; out[key]["kernel_only_replica_steps_per_s"] = r["kernel_only_replica_steps_per_s"]
+        except Exception as e:                      # an extra must never cost the main line
+            out[key] = {"error": repr(e)[:300]}
+        out[key]["wall_s"] = round(time.perf_counter() - t0, 1)
+    return out
 
 
 # ------------------------------------------------------------------------------------------------------------------ config 4
@@ -460,7 +516,7 @@ def run_eval_reference(args):
         "e2e": {"value": val, "unit": C4_UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
-def run_eval(args):
+def run_eval(args, emit=True):
     import torch
     import torch.distributed as dist
     from paper_2508_15522_b200 import api, shard
@@ -468,7 +524,7 @@ def run_eval(args):
     world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local)
-    if world > 1:
+    if world > 1 and not dist.is_initialized():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     stream = torch.cuda.current_stream()
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -589,19 +645,23 @@ def run_eval(args):
 
     l2 = l2_probe(sb)
     kern_ms = float(np.mean(ts))
+    tkey = "config4" if args.c4_grid == "config1" else "config4_%s" % args.c4_grid.lower()
+    if args.order == "sorted":
+        tkey += "_sorted"
     fits, ach, peak = roof(sb, n, kern_ms, l2)
     traffic = None
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get("config4")
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(tkey)
     except Exception:
         pass
     roofline = {"bound": "l2" if fits else "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
-                "kernel": {"fp32": "k_eval_coop (warp-cooperative tricubic gather)", "half": "k_eval_half (tricubic, fp16 coefficients)",
+                "kernel": {"fp32": "k_eval_coop (warp-cooperative LDG gather)" if fits or args.variant == 2 else
+                                   "k_eval_tma (one 3-D TMA box per point) for scattered points / k_eval_coop for sorted points, chosen on the device", "half": "k_eval_half (tricubic, fp16 coefficients)",
                            "trilinear": "k_eval_trilinear (8-corner foil, E and F tables)"}[args.c4_store], "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
                 "bytes_per_eval": bpe, "evals_per_launch": n, "io_bytes_per_eval_hbm": C4_IO_BYTES,
                 "io_stream_gbs": n * float(C4_IO_BYTES) / (kern_ms * 1e-3) / 1e9,
                 "peak_source": "L2 read bandwidth measured in this run by gridff_probe_read" if fits else hbm_src,
-                "l2_probe_gbs": l2, "hbm_peak_gbs": hbm_peak, "frac_of_hbm_peak": ach / hbm_peak}
+                "l2_probe_gbs": l2, "hbm_peak_gbs": hbm_peak, "frac_of_hbm_peak": ach / hbm_peak, "ncu": ncu_facts(tkey)}
 
     sweep = None
     if args.sweep:
@@ -644,14 +704,17 @@ def run_eval(args):
         cpu = {"value": n_s / t, "unit": C4_UNIT, "cores": orc.num_threads(), "kind": "oracle",
                "sample": "the first 2^%d of the 2^%d points (%.2f s), grid resident, fp64" % (int(np.log2(n_s)), args.log2_points, t)}
 
-    print(json.dumps({
+    line = ({
         "metric": C4_METRIC, "value": value, "unit": C4_UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "config4: 2^%d uniformly random points, %s, 3-channel E + analytic gradient" % (args.log2_points, name),
                    "grid": list(dims), "store": args.c4_store, "store_bytes": sb, "points_per_gpu": n, "order": args.order, "parallelism": "points only (no collective)",
                    "l2_flush_between_steps": True, "step": "gridff_eval over all points (grid built before the timed region)"},
         "clocks": clocks, "e2e": {"value": e2e_value, "unit": C4_UNIT, "h2d_bytes_per_step": n * 28, "d2h_bytes_per_step": n * 16},
-        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "sweep": sweep}))
+        "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "sweep": sweep})
+    if not emit:
+        return line
+    print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
 
