@@ -44,9 +44,11 @@ def parse():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-also", action="store_true", help="default (config 1, N = 1) run: skip the short extra measurements of configs 2, 3 and 4 reported under 'also'")
-    ap.add_argument("--mode", default="run", choices=["run", "langevin", "hopping", "scan"],
+    ap.add_argument("--mode", default="run", choices=["run", "langevin", "hopping", "scan", "drag"],
                     help="SURVEY §8(f) rows on the chosen replica config: langevin = kind 2 instead of the config's integrator; hopping = "
-                         "gridff_minima_hopping cycles (1000 Langevin steps at 300 K + FIRE); scan = gridff_run_scan lift of one held atom")
+                         "gridff_minima_hopping cycles (1000 Langevin steps at 300 K + FIRE); scan = gridff_run_scan lift of one held atom; "
+                         "drag = the paper's defect protocol (L184, L200-202): a Na-Cl vacancy pair is cut into the config's substrate and every "
+                         "replica drags its held atom across it in 40 steps of 0.1 A, relaxing at each (use with --config 3 for the 20x20 cell)")
     ap.add_argument("--log2-points", type=int, default=26, help="config 4: number of interpolation points = 2^k")
     ap.add_argument("--order", default="random", choices=["random", "sorted"], help="config 4: point order (sorted = Morton order of the cell)")
     ap.add_argument("--c4-grid", default="config1", help="config 4: 'config1' (the 113 x 113 x 100 NaCl grid) or NXxNYxNZ synthetic sweep grid")
@@ -181,6 +183,9 @@ def run_f_rows(args):
     cfg, md, dims, name = workload(args)
     d, topo, sub = cfg["desc"], cfg["topo"], cfg["sub"]
     n_rep, n_at = cfg["n_rep"], int(topo["n_atoms"])
+    if args.mode == "drag":
+        sub, removed = inputs.vacancy_pair(sub, d["Lx"], d["Ly"])
+        cfg["pos"] = inputs.drag_starts(topo, n_rep, n_at - 1, removed[:, :2].mean(axis=0) - [2.0, 0.0], 3.3, 1.0, cfg["seed"] + 30)
     g = api.gridff_build_grid(api.make_desc(d["Lx"], d["Ly"], d["z_ref"], d["z_lo"], d["z_hi"], d["spacing"], d["alpha"], d["channels"], r_cut=d["r_cut"], l2_persist=1),
                               sub["pos"], sub["e"], sub["R"], sub["q"])
     mol = api.gridff_create_molecule(topo, api.gridff_atom_coefs(d["alpha"], topo["grid_e"], topo["grid_R"], topo["q"]))
@@ -209,18 +214,23 @@ def run_f_rows(args):
             units = n_rep * cycles                       # hops
             extra = {"cycles": cycles, "md_steps": 1000, "relax_cap": 5000, "stats_per_cycle[candidates,new,dropped,library]": st.tolist()}
         else:
-            n_scan = 20
-            integ = api.make_integrator("fire", 2000, 1.0, f_tol=2e-3, dt_max=10.0, max_step=0.05, n_scan=n_scan, fixed=(n_at - 1,), scan_dx=(0.0, 0.0, 0.1))
+            n_scan = 40 if args.mode == "drag" else 20
+            sdx = (0.1, 0.0, 0.0) if args.mode == "drag" else (0.0, 0.0, 0.1)
+            integ = api.make_integrator("fire", 2000, 1.0, f_tol=2e-3, dt_max=10.0, max_step=0.05, n_scan=n_scan, fixed=(n_at - 1,), scan_dx=sdx)
             a.record(stream); out = api.gridff_run_scan(g, mol, integ, d_pos, d_vel); b.record(stream); b.synchronize()
             units = int(out["status"][:, 0].sum().item())        # FIRE iterations really taken
             extra = {"n_scan": n_scan, "points_converged_frac": float(out["scan"][..., 2].mean().item()), "scan_points_per_s": None}
+            if args.mode == "drag":
+                e_s = out["scan"][..., 0].mean(dim=0).cpu().numpy()
+                extra.update(substrate_atoms=int(len(sub["pos"])), removed_sites=removed.tolist(),
+                             mean_E_along_path_eV=[round(float(v), 4) for v in e_s[::4]])
         if it >= max(args.warmup, 3):
             ts.append(a.elapsed_time(b))
     ms = float(np.mean(ts))
-    if args.mode == "scan":
+    if args.mode in ("scan", "drag"):
         extra["scan_points_per_s"] = n_rep * extra["n_scan"] / (ms * 1e-3)
-    unit = {"langevin": "replica-steps/s", "hopping": "hops/s", "scan": "replica-steps/s"}[args.mode]
-    print(json.dumps({"metric": {"langevin": "replica_md_steps_per_s", "hopping": "minima_hops_per_s", "scan": "replica_md_steps_per_s"}[args.mode],
+    unit = {"langevin": "replica-steps/s", "hopping": "hops/s", "scan": "replica-steps/s", "drag": "replica-steps/s"}[args.mode]
+    print(json.dumps({"metric": {"langevin": "replica_md_steps_per_s", "hopping": "minima_hops_per_s", "scan": "replica_md_steps_per_s", "drag": "replica_md_steps_per_s"}[args.mode],
                       "value": units / (ms * 1e-3), "unit": unit, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms,
                       "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                       "config": {"workload": "%s [mode %s]" % (name, args.mode), "n_replicas_per_gpu": n_rep, "atoms": n_at, "l2_flush_between_steps": True},

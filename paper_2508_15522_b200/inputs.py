@@ -48,6 +48,32 @@ def rocksalt_slab(n_sites, n_layers, d, q):
     return sub, n_sites * d, n_sites * d
 
 
+def vacancy_pair(sub, Lx, Ly):
+    """The paper's neutral defect ("removing one Na and one Cl atoms next to each other from the topmost atomic layer"): the
+    top-layer atom nearest the cell centre and its nearest oppositely charged top-layer neighbour are removed.  Returns (substrate without
+    the pair, positions [2][3] of the removed atoms)."""
+    pos, q = np.asarray(sub["pos"]), np.asarray(sub["q"])
+    top = np.where(np.abs(pos[:, 2] - pos[:, 2].max()) < 1e-9)[0]
+    first = top[np.argmin(np.linalg.norm(pos[top, :2] - [Lx / 2, Ly / 2], axis=1))]
+    others = [t for t in top if t != first and q[t] == -q[first]]
+    second = others[int(np.argmin([np.linalg.norm(pos[t, :2] - pos[first, :2]) for t in others]))]
+    keep = np.array([i for i in range(len(pos)) if i not in (first, second)])
+    out = {k: np.ascontiguousarray(np.asarray(v)[keep]) for k, v in sub.items() if k != "elements"}
+    return out, pos[[first, second]].copy()
+
+
+def drag_starts(topo, n_rep, held, start_xy, z_above, spread, seed):
+    """replicas for a drag scan: the molecule flat (template orientation) `z_above` over z = 0, translated so that its
+    held atom sits at start_xy + U(-spread, spread) in x and y; float32 [n_rep][n][3]"""
+    rng = np.random.default_rng(seed)
+    ref = np.asarray(topo["ref_pos"], np.float64)
+    out = np.repeat(ref[None], n_rep, 0)
+    out[..., 2] += z_above - ref[held, 2]
+    shift = np.asarray(start_xy)[None, :] + rng.uniform(-spread, spread, (n_rep, 2)) - ref[held, :2][None, :]
+    out[..., :2] += shift[:, None, :]
+    return out.astype(np.float32)
+
+
 # ----------------------------------------------------------------------------- topology helpers
 
 def _neighbors(n, bonds):

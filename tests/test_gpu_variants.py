@@ -91,14 +91,9 @@ def test_defective_substrate_grid_and_eval(api, orc):
     the topmost atomic layer)"): the build takes any neutral periodic substrate.  4x4-site, 3-layer slab with a Na-Cl vacancy pair in
     the top layer: coefficients at half an fp32 ulp of the oracle's, interpolation within the north_star tolerances over the defect."""
     sub, Lx, Ly = inputs.rocksalt_slab(4, 3, 2.82, 0.7)
-    top = np.where(np.abs(sub["pos"][:, 2] - sub["pos"][:, 2].max()) < 1e-9)[0]
-    c = np.array([Lx / 2, Ly / 2])
-    first = top[np.argmin(np.linalg.norm(sub["pos"][top, :2] - c, axis=1))]
-    others = [t for t in top if t != first and sub["q"][t] == -sub["q"][first]]
-    second = others[int(np.argmin([np.linalg.norm(sub["pos"][t, :2] - sub["pos"][first, :2]) for t in others]))]
-    keep = np.array([i for i in range(len(sub["pos"])) if i not in (first, second)])
-    sub = {k: np.ascontiguousarray(np.asarray(v)[keep]) for k, v in sub.items() if k != "elements"}
-    assert abs(sub["q"].sum()) < 1e-12 and len(keep) == 46
+    sub, removed = inputs.vacancy_pair(sub, Lx, Ly)
+    first = 0
+    assert abs(sub["q"].sum()) < 1e-12 and len(sub["pos"]) == 46
     desc = inputs.grid_desc(Lx, Ly, 0.0, 1.5, 6.5, 0.2, 1.6, [inputs.PAULI, inputs.LONDON, inputs.COULOMB])
     og, _ = oracle_grid(orc, sub, desc)
     g = gpu_grid(api, sub, desc)
@@ -115,7 +110,7 @@ def test_defective_substrate_grid_and_eval(api, orc):
     Eo, Fo, Vc, _ = orc.interp(og, pos, cf, channels=True)
     den = np.sum(np.abs(cf[:, :3].astype(np.float64) * Vc), axis=1)
     assert (np.abs(E.cpu().numpy() - Eo) / den).max() <= 1e-5 and np.abs(F.cpu().numpy() - Fo).max() <= 1e-4
-    v0 = inputs.rocksalt_slab(4, 3, 2.82, 0.7)[0]["pos"][first]                  # the removed atom's site
+    v0 = removed[first]                                                        # the removed atom's site
     p2 = np.array([[v0[0], v0[1], 2.0], [(v0[0] + 2 * 2.82) % Lx, v0[1], 2.0]])
     V = orc.interp(og, p2, np.array([[1.0, 0, 0, 0]] * 2))[0]
     assert abs(V[0] - V[1]) > 1e-3 * abs(V[1])
