@@ -52,8 +52,9 @@ def parse():
     ap.add_argument("--log2-points", type=int, default=26, help="config 4: number of interpolation points = 2^k")
     ap.add_argument("--order", default="random", choices=["random", "sorted"], help="config 4: point order (sorted = Morton order of the cell)")
     ap.add_argument("--c4-grid", default="config1", help="config 4: 'config1' (the 113 x 113 x 100 NaCl grid) or NXxNYxNZ synthetic sweep grid")
-    ap.add_argument("--c4-store", default="fp32", choices=["fp32", "half", "trilinear"],
-                    help="config 4: coefficient store read by gridff_eval: the fp32 spline (default), fp16 coefficients, or the paper's trilinear foil (SURVEY §8(f)3)")
+    ap.add_argument("--c4-store", default="fp32", choices=["fp32", "half", "trilinear", "bricks", "bricks2", "bricks8"],
+                    help="config 4: coefficient store read by gridff_eval: the fp32 spline z-fastest (default), fp16 coefficients, the paper's trilinear foil "
+                         "(SURVEY §8(f)3), or the fp32 spline in 2x2x2-node bricks of 128 B, 1 / 2 / 8 shifted copies (the layouts for stores beyond the L2)")
     ap.add_argument("--sweep", action="store_true", help="config 4: also time the grid-size x order sweep (32^3 ... 512x512x256)")
     return ap.parse_args()
 
@@ -450,9 +451,10 @@ def also_entries(args):
             ("config4_random", dict(config=4, order="random", c4_grid="config1", log2_points=26)),
             ("config4_sorted", dict(config=4, order="sorted", c4_grid="config1", log2_points=26)),
             ("config4_hbm_512x512x256_random", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25)),
-            ("config4_hbm_512x512x256_sorted", dict(config=4, order="sorted", c4_grid="512x512x256", log2_points=25))]
+            ("config4_hbm_512x512x256_sorted", dict(config=4, order="sorted", c4_grid="512x512x256", log2_points=25)),
+            ("config4_hbm_512x512x256_random_bricks8", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25, c4_store="bricks8"))]
     for key, kw in todo:
-        a = argparse.Namespace(**dict(base, c4_store="fp32", sweep=False, **kw))
+        a = argparse.Namespace(**dict(dict(base, c4_store="fp32", sweep=False), **kw))
         t0 = time.perf_counter()
         try:
             r = run_eval(a, emit=False) if a.config == 4 else run_gridff(a, emit=False)
@@ -550,7 +552,8 @@ def run_eval(args, emit=True):
         g0 = make_grid_fp32(desc, dims, sub)
         if store == "fp32":
             return g0
-        gd_ = api.gridff_grid_derive(g0, api.LAYOUT_HALF if store == "half" else api.LAYOUT_TRILINEAR)
+        gd_ = api.gridff_grid_derive(g0, {"half": api.LAYOUT_HALF, "trilinear": api.LAYOUT_TRILINEAR, "bricks": api.LAYOUT_MBRICK,
+                                          "bricks2": api.LAYOUT_MBRICK2, "bricks8": api.LAYOUT_MBRICK8}[store])
         torch.cuda.synchronize()
         g0.free()
         return gd_
@@ -597,7 +600,7 @@ def run_eval(args, emit=True):
     n = 1 << args.log2_points
     g = make_grid(desc, dims, sub, args.c4_store)
     sb = g.store.numel()
-    bpe = BYTES_PER_EVAL if args.c4_store == "fp32" else 512          # half: 64 nodes x 8 B; trilinear foil: 8 nodes x 64 B
+    bpe = 512 if args.c4_store in ("half", "trilinear") else BYTES_PER_EVAL          # half: 64 nodes x 8 B; trilinear foil: 8 nodes x 64 B
     pos, coef = make_points(desc, dims, n, shard.rank_seed(1004, rank))
     d_pos, d_coef = torch.from_numpy(pos).cuda(), torch.from_numpy(coef).cuda()
     z0 = desc["z_ref"] + desc["z_lo"]
@@ -658,6 +661,8 @@ def run_eval(args, emit=True):
     tkey = "config4" if args.c4_grid == "config1" else "config4_%s" % args.c4_grid.lower()
     if args.order == "sorted":
         tkey += "_sorted"
+    if args.c4_store != "fp32":
+        tkey += "_" + args.c4_store
     fits, ach, peak = roof(sb, n, kern_ms, l2)
     traffic = None
     try:
@@ -667,7 +672,9 @@ def run_eval(args, emit=True):
     roofline = {"bound": "l2" if fits else "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": traffic,
                 "kernel": {"fp32": "k_eval_coop (warp-cooperative LDG gather)" if fits or args.variant == 2 else
                                    "k_eval_tma (one 3-D TMA box per point) for scattered points / k_eval_coop for sorted points, chosen on the device", "half": "k_eval_half (tricubic, fp16 coefficients)",
-                           "trilinear": "k_eval_trilinear (8-corner foil, E and F tables)"}[args.c4_store], "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
+                           "trilinear": "k_eval_trilinear (8-corner foil, E and F tables)",
+                           "bricks": "k_eval_bricks (warp-cooperative LDG gather over 2x2x2-node bricks)", "bricks2": "k_eval_bricks (2 shifted copies)",
+                           "bricks8": "k_eval_tma<bricks> (one 5-D TMA box = 8 whole 128-byte lines per point; 8 shifted copies)"}[args.c4_store], "kernel_ms": kern_ms, "kernel_share_of_step": kern_ms / ms_per_step,
                 "bytes_per_eval": bpe, "evals_per_launch": n, "io_bytes_per_eval_hbm": C4_IO_BYTES,
                 "io_stream_gbs": n * float(C4_IO_BYTES) / (kern_ms * 1e-3) / 1e9,
                 "peak_source": "L2 read bandwidth measured in this run by gridff_probe_read" if fits else hbm_src,
@@ -684,11 +691,11 @@ def run_eval(args, emit=True):
             perm = inputs.morton_order(dp0, gdesc["Lx"], gdesc["Ly"], gdesc["z_ref"] + gdesc["z_lo"], gdims[0], gdims[1], gdesc["spacing"], xp=torch)
             dp1, dc1 = dp0[perm].contiguous(), dc0[perm].contiguous()
             del perm, p_, c_
-            for store in ("fp32", "half", "trilinear"):
+            for store in ("fp32", "half", "trilinear", "bricks", "bricks2", "bricks8"):
                 gg = make_grid(gdesc, gdims, gsub, store)
                 gsb = gg.store.numel()
                 gl2 = l2_probe(gsb) if gsb < (100 << 20) else l2
-                sbpe = BYTES_PER_EVAL if store == "fp32" else 512
+                sbpe = 512 if store in ("half", "trilinear") else BYTES_PER_EVAL
                 for order, dp, dc in (("random", dp0, dc0), ("sorted", dp1, dc1)):
                     t = float(np.mean(time_eval(gg, dp, dc, d_E, d_F, 3, 2)))
                     f_, a_, pk = roof(gsb, n, t, gl2, sbpe)

@@ -51,8 +51,17 @@ typedef enum {
     GRIDFF_LAYOUT_BRICK = 1,  /* 4x4x4-node bricks of 1 KB, bricks in [x][y][z] order, x/y halo                     */
     /* derived stores (gridff_grid_derive; gridff_eval only — SURVEY.md §8(f) row 3): */
     GRIDFF_LAYOUT_HALF = 2,   /* ZFAST with the 4 coefficients of a node rounded to fp16 (8 B per node), fp32 arithmetic */
-    GRIDFF_LAYOUT_TRILINEAR = 3 /* the trilinear foil of PAPER.md:L118-120, L140: per node V and the three gradient components for
+    GRIDFF_LAYOUT_TRILINEAR = 3, /* the trilinear foil of PAPER.md:L118-120, L140: per node V and the three gradient components for
                                    each channel (4 x float4 = 64 B), each interpolated independently over the 8 cell corners   */
+    /* derived fp32 stores for grids that do not fit the L2 (the HBM-bound gather): the same coefficients in
+       2x2x2-node bricks of 128 B (one memory line), bricks in [x][y][z] order.  The 4x4x4 stencil of PAPER.md:L136 then touches
+       whole lines only; the results are bit-identical to the z-fastest store's (variant 2). */
+    GRIDFF_LAYOUT_MBRICK = 4,    /* one copy: a stencil touches 8 / 12 / 18 / 27 lines by the parity of its corner (15.6 on average; the
+                                   z-fastest store: 22 partly used lines)                                                         */
+    GRIDFF_LAYOUT_MBRICK2 = 5,   /* two copies, the second anchored one node further in x, y and z: the better aligned copy is read
+                                   (8 or 12 lines, 11 on average), 2 x the memory                                                  */
+    GRIDFF_LAYOUT_MBRICK8 = 6    /* eight copies, one per parity of the corner: EVERY stencil is exactly 8 whole lines = the 1024
+                                   algorithmic bytes, 8 x the memory (sized for 180 GB of HBM: a 1 GB grid becomes 8.7 GB)        */
 } gridff_layout;
 
 typedef struct {
@@ -109,6 +118,8 @@ int gridff_free_grid(gridff_grid* grid);
  *   GRIDFF_LAYOUT_TRILINEAR  node values V_c = the parent spline at the node and G_c = its analytic gradient there (R20);
  *                            gridff_eval then returns E = sum_c coef_c lerp(V_c), F = -sum_c coef_c lerp(G_c) ("the force components
  *                            and energy were stored and interpolated independently", L120), cell and domain rules as for the spline.
+ *   GRIDFF_LAYOUT_MBRICK / MBRICK2 / MBRICK8   the parent's fp32 coefficients re-laid in 2x2x2-node bricks, 1 / 2 / 8 copies (see
+ *                            gridff_layout); needs nx + 3, ny + 3 <= 2047 and nz <= 1023; gridff_eval returns the parent's numbers bit for bit.
  * d_store (>= gridff_derive_bytes) stays the caller's; the handle is freed with gridff_free_grid.                          */
 size_t gridff_derive_bytes(const gridff_grid* parent, int layout);
 int gridff_grid_derive(const gridff_grid* parent, int layout, void* d_store, size_t store_bytes, void* cuda_stream, gridff_grid** out);
@@ -131,7 +142,8 @@ int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const 
 /* Same with an explicit kernel variant (layout / gather study): 0 = library default, 1 = one thread per point
  * (64 independent 16-byte loads), 2 = warp-cooperative row gather, 3 = one 3-D TMA box (cp.async.bulk.tensor, 1 KB) per point into shared
  * memory (z-fastest fp32 stores only; GRIDFF_EUNSUPPORTED when the driver has no tensor-map entry point).  Variants 2 and 3 return
- * bit-identical results.  A brick-layout grid always uses its own kernel. */
+ * bit-identical results.  A brick-layout grid always uses its own kernel.  Micro-brick stores (GRIDFF_LAYOUT_MBRICK*): 0 / 2 = the
+ * warp-cooperative gather over bricks, 3 = one 5-D TMA box {brick, 2, 2, 2, copy} per point (MBRICK8 only; the default there). */
 int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
                         float* d_E, float* d_F, int variant, void* cuda_stream);
 

@@ -21,7 +21,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gridff_oracle.c")
-_LIB = os.path.join(_HERE, "libgridff_oracle.so")
+# GRIDFF_ORACLE_SANITIZE=1: the same source built with -fsanitize=address,undefined into its own library (run the CPU pins under
+# LD_PRELOAD=$(gcc -print-file-name=libasan.so); profiles/r2_sanitizers.md)
+_SAN = os.environ.get("GRIDFF_ORACLE_SANITIZE", "") == "1"
+_LIB = os.path.join(_HERE, "libgridff_oracle_san.so" if _SAN else "libgridff_oracle.so")
 _lib = None
 
 KE = 14.3996454784
@@ -32,7 +35,8 @@ KB = 8.617333262e-5
 def build(force=False):
     """Compile the oracle with gcc (-O2 -fopenmp).  Building the checker is not using it."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if _SAN else ["-O2"]
+        subprocess.check_call(["gcc"] + flags + ["-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
     return _LIB
 
 

@@ -224,10 +224,12 @@ def gridff_grid_from_samples(desc, d_samples, stream=None):
 
 
 LAYOUT_HALF, LAYOUT_TRILINEAR = 2, 3
+LAYOUT_MBRICK, LAYOUT_MBRICK2, LAYOUT_MBRICK8 = 4, 5, 6       # 2x2x2-node bricks, 1 / 2 / 8 shifted copies (stores beyond the L2)
 
 
 def gridff_grid_derive(parent, layout, stream=None):
-    """derived store for the interpolation trade study: LAYOUT_HALF (fp16 coefficients) or LAYOUT_TRILINEAR (the paper's foil); gridff_eval only."""
+    """derived store: LAYOUT_HALF (fp16 coefficients), LAYOUT_TRILINEAR (the paper's foil) or LAYOUT_MBRICK / MBRICK2 / MBRICK8 (the fp32
+    coefficients in 128-byte bricks for stores beyond the L2); gridff_eval only."""
     nbytes = int(_lib.gridff_derive_bytes(parent.handle, int(layout)))
     store = _alloc(nbytes)
     out = C.c_void_p(None)

@@ -2,7 +2,9 @@
 //   GRIDFF_LAYOUT_HALF       fp16 coefficients (8 B per node), tricubic B-spline with fp32 accumulation
 //   GRIDFF_LAYOUT_TRILINEAR  the trilinear foil the paper compares against ("the force components (Fx, Fy, Fz) and
 //                            energy E were stored and interpolated independently"; L140: tricubic "only about two times slower")
-// Both are built from a ZFAST fp32 grid and are read by gridff_eval only.
+//   GRIDFF_LAYOUT_MBRICK*    the fp32 coefficients in 2 x 2 x 2-node bricks of one 128-byte line, 1 / 2 / 8 shifted copies: the layout for
+//                            stores that exceed the L2, where DRAM moves whole lines and the z-fastest rows waste 1.7 of every 2.7 bytes
+// All are built from a ZFAST fp32 grid and are read by gridff_eval only.
 #include "gridff_interp.cuh"
 #include <cuda_fp16.h>
 #include <string.h>
@@ -127,9 +129,78 @@ __global__ void __launch_bounds__(256) k_eval_trilinear(GridGeom g, int nzt, lon
     else if (F) F[3 * p + (j - 1)] = -out;
 }
 
+// ---- micro-brick stores (addressing: gridff_interp.cuh) ----------------------------------------------------------------------------------
+__global__ void k_to_bricks(GridGeom parent, GridGeom g, float4* __restrict__ dst) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= g.copy_stride * g.n_copies) return;
+    const int copy = (int)(k / g.copy_stride);
+    const long long r = k - (long long)copy * g.copy_stride;
+    const int in = (int)(r & 7); long long b = r >> 3;
+    const int bz = (int)(b % g.nbz); b /= g.nbz;
+    const int by = (int)(b % g.nby), bx = (int)(b / g.nby);
+    const int sh = brick_shift_bits(g.n_copies, copy);
+    const int X = 2 * bx - ((sh >> 2) & 1) + ((in >> 2) & 1), Y = 2 * by - ((sh >> 1) & 1) + ((in >> 1) & 1), Z = 2 * bz - (sh & 1) + (in & 1);
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (X >= 0 && X < parent.sx && Y >= 0 && Y < parent.sy && Z >= 0 && Z < parent.nzp) v = parent.store[((size_t)X * parent.sy + Y) * parent.nzp + Z];
+    dst[k] = v;
+}
+
+// k_eval_coop over bricks: a warp owns 32 points, gathers each stencil cooperatively (lane <-> node as over the z-fastest store, so the folded
+// tile, the contraction and the results are the same bit for bit), every lane then contracts its own point
+__global__ void __launch_bounds__(kWarps * 32) k_eval_bricks(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
+                                                             float* __restrict__ E, float* __restrict__ F) {
+    __shared__ __align__(16) float s_tile[kWarps][32 * 64];
+    __shared__ __align__(16) float4 s_cf[kWarps][32];
+    __shared__ unsigned s_corner[kWarps][32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const long long p = ((long long)blockIdx.x * kWarps + w) * 32 + lane;
+    Stencil s; s.base = kNoStencil; s.tx = s.ty = s.tz = 0.f;
+    float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
+    int ix = 0, iy = 0, iz = 0;
+    if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz); cf = coef[p]; }
+    s_corner[w][lane] = s.base == kNoStencil ? kNoStencil : pack_corner(ix, iy, iz - 1);
+    s_cf[w][lane] = cf;
+    __syncwarp();
+    float* tile = s_tile[w];
+    if (warp_points_are_local(ix, iy, iz, s.base != kNoStencil, lane)) {
+#pragma unroll 8
+        for (int q = 0; q < 32; ++q) {
+            const unsigned c = s_corner[w][q];
+            if (c != kNoStencil) gather_bricks<false>(g, c, s_cf[w][q], lane, q, tile);
+        }
+    } else {
+#pragma unroll 8
+        for (int q = 0; q < 32; ++q) {
+            const unsigned c = s_corner[w][q];
+            if (c != kNoStencil) gather_bricks<true>(g, c, s_cf[w][q], lane, q, tile);
+        }
+    }
+    __syncwarp();
+    if (p >= n) return;
+    float e, fx, fy, fz;
+    interp_tile(g, s, lane, tile, e, fx, fy, fz);
+    if (E) E[p] = e;
+    if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
+}
+
+inline int brick_copies(int layout) { return layout == GRIDFF_LAYOUT_MBRICK8 ? 8 : layout == GRIDFF_LAYOUT_MBRICK2 ? 2 : layout == GRIDFF_LAYOUT_MBRICK ? 1 : 0; }
+inline void brick_extents(const GridGeom& P, int& nbx, int& nby, int& nbz) { nbx = (P.sx >> 1) + 1; nby = (P.sy >> 1) + 1; nbz = (P.nzp >> 1) + 1; }
+
 }  // namespace
 
 namespace gridff {
+
+int eval_bricks(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, int variant, cudaStream_t st) {
+    const GridGeom& G = grid->geom;
+    if (variant != 0 && variant != 2 && variant != 3) { set_error("micro-brick stores have variants 0, 2 (LDG gather) and 3 (TMA, 8 copies)"); return GRIDFF_EINVAL; }
+    if (variant == 3 && !(G.n_copies == 8 && grid->tmap_ok)) { set_error("the TMA variant needs the 8-copy micro-brick store and a tensor map"); return GRIDFF_EUNSUPPORTED; }
+    if (variant == 3 || (variant == 0 && G.n_copies == 8 && grid->tmap_ok && n >= 4096)) return eval_tma(grid, n, d_pos, d_coef, d_E, d_F, nullptr, st);
+    const long long per_block = kWarps * 32;
+    cudaError_t e = launch_with_window(grid, k_eval_bricks, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    count_launch();
+    if (e != cudaSuccess) return cuda_fail(e, "gridff_eval (micro-brick store) launch");
+    return GRIDFF_OK;
+}
 
 int eval_derived(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st) {
     const GridGeom& G = grid->geom;
@@ -155,6 +226,7 @@ size_t gridff_derive_bytes(const gridff_grid* parent, int layout) {
     const GridGeom& G = parent->geom;
     if (layout == GRIDFF_LAYOUT_HALF) return (size_t)G.sx * G.sy * G.nzp * 8;
     if (layout == GRIDFF_LAYOUT_TRILINEAR) return (size_t)(G.nx + 1) * (G.ny + 1) * ((G.nz + 1) & ~1) * 64;
+    if (brick_copies(layout)) { int bx, by, bz; brick_extents(G, bx, by, bz); return (size_t)brick_copies(layout) * bx * by * bz * 128; }
     return 0;
 }
 
@@ -162,7 +234,10 @@ int gridff_grid_derive(const gridff_grid* parent, int layout, void* d_store, siz
     if (!parent || !out) { set_error("parent / out is NULL"); return GRIDFF_EINVAL; }
     *out = nullptr;
     if (parent->geom.layout != GRIDFF_LAYOUT_ZFAST) { set_error("derived stores are built from a z-fastest fp32 grid"); return GRIDFF_EUNSUPPORTED; }
-    if (layout != GRIDFF_LAYOUT_HALF && layout != GRIDFF_LAYOUT_TRILINEAR) { set_error("unknown derived layout %d", layout); return GRIDFF_EINVAL; }
+    if (layout != GRIDFF_LAYOUT_HALF && layout != GRIDFF_LAYOUT_TRILINEAR && !brick_copies(layout)) { set_error("unknown derived layout %d", layout); return GRIDFF_EINVAL; }
+    if (brick_copies(layout) && (parent->geom.sx > 2047 || parent->geom.sy > 2047 || parent->geom.nzp > 1023)) {
+        set_error("micro-brick stores need nx + 3, ny + 3 <= 2047 and nz <= 1023"); return GRIDFF_EUNSUPPORTED;
+    }
     const size_t need = gridff_derive_bytes(parent, layout);
     if (!d_store || store_bytes < need) { set_error("derived store buffer too small: %zu < %zu", store_bytes, need); return GRIDFF_ESIZE; }
     if ((uintptr_t)d_store & 255) { set_error("d_store must be 256-byte aligned"); return GRIDFF_EINVAL; }
@@ -172,7 +247,7 @@ int gridff_grid_derive(const gridff_grid* parent, int layout, void* d_store, siz
         const long nn = (long)G.sx * G.sy * G.nzp;
         k_to_half<<<blocks_for(nn, 256), 256, 0, st>>>(G.store, nn, (uint2*)d_store);
         GRIDFF_LAUNCH_CHECK("k_to_half");
-    } else {
+    } else if (layout == GRIDFF_LAYOUT_TRILINEAR) {
         const int nzt = (G.nz + 1) & ~1;
         const long nn = (long)(G.nx + 1) * (G.ny + 1) * nzt;
         k_to_trilinear<<<blocks_for(nn, 128), 128, 0, st>>>(G, nzt, (float4*)d_store);
@@ -184,6 +259,19 @@ int gridff_grid_derive(const gridff_grid* parent, int layout, void* d_store, siz
     g->geom.layout = layout;
     g->geom.store = (const float4*)d_store;
     g->store_bytes = need;
+    g->tmap_ok = 0;
+    if (brick_copies(layout)) {
+        GridGeom& B = g->geom;
+        brick_extents(G, B.nbx, B.nby, B.nbz);
+        B.n_copies = brick_copies(layout);
+        B.copy_stride = (long long)B.nbx * B.nby * B.nbz * 8;
+        const long long nn = B.copy_stride * B.n_copies;
+        k_to_bricks<<<(unsigned)((nn + 255) / 256), 256, 0, st>>>(G, B, (float4*)d_store);
+        count_launch();
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) { delete g; return cuda_fail(e, "k_to_bricks"); }
+        if (B.n_copies == 8 && make_tensor_map(g) != GRIDFF_OK) g->tmap_ok = 0;      // variant 3 then reports it; the LDG gather serves
+    }
     *out = g;
     return GRIDFF_OK;
 }

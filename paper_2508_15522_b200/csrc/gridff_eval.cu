@@ -193,6 +193,7 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e;
     if (G.layout == GRIDFF_LAYOUT_HALF || G.layout == GRIDFF_LAYOUT_TRILINEAR) return eval_derived(grid, n, d_pos, d_coef, d_E, d_F, st);
+    if (G.n_copies > 0) return eval_bricks(grid, n, d_pos, d_coef, d_E, d_F, variant, st);
     if (G.layout == GRIDFF_LAYOUT_BRICK) {
         e = launch_with_window(grid, k_eval_brick, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
     } else if (variant == 1) {

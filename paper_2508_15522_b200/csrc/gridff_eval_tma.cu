@@ -49,24 +49,40 @@ __device__ __forceinline__ void tma_box(void* dst, const CUtensorMap* map, int c
     asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
                  ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
+// 8-copy micro-brick store: one {32 floats = a brick, 2, 2, 2, 1} box: (0, brick z, brick y, brick x, copy) — 8 whole 128-byte lines
+__device__ __forceinline__ void tma_box5(void* dst, const CUtensorMap* map, int bz, int by, int bx, int copy, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6, %7}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(smem_u32(bar)), "r"(0), "r"(bz), "r"(by), "r"(bx), "r"(copy) : "memory");
+}
 
-struct Pt { unsigned base; float tx, ty, tz; int c0, c1, c2; float4 cf; };
+// base: the stencil's corner in the z-fastest store (BRICKS: the packed corner for gather_bricks); kNoStencil = above the domain
+struct Pt { unsigned base; float tx, ty, tz; int c0, c1, c2, c3; float4 cf; };
 
+template <bool BRICKS>
 __device__ __forceinline__ Pt load_point(const GridGeom& g, long long p, long long n, const float* __restrict__ pos, const float4* __restrict__ coef) {
-    Pt q; q.base = kNoStencil; q.tx = q.ty = q.tz = 0.f; q.c0 = q.c1 = q.c2 = 0; q.cf = make_float4(0.f, 0.f, 0.f, 0.f);
+    Pt q; q.base = kNoStencil; q.tx = q.ty = q.tz = 0.f; q.c0 = q.c1 = q.c2 = q.c3 = 0; q.cf = make_float4(0.f, 0.f, 0.f, 0.f);
     if (p < n) {
         int ix, iy, iz;
         cell_periodic(pos[3 * p], g.inv_hx_hi, g.inv_hx_lo, g.fnx, g.inv_nx, ix, q.tx);
         cell_periodic(pos[3 * p + 1], g.inv_hy_hi, g.inv_hy_lo, g.fny, g.inv_ny, iy, q.ty);
         if (cell_z(pos[3 * p + 2], g, iz, q.tz)) {
-            q.base = (unsigned)corner_zfast(g, ix, iy, iz);        // same validity flag and offsets as the LDG kernels
-            q.c0 = 4 * (iz - 1); q.c1 = iy; q.c2 = ix;             // stored index s holds node s - 1: the stencil corner (ix-1, iy-1) is stored at (ix, iy)
+            if (BRICKS) {
+                // corner (ix, iy, iz - 1) in stored indices; the copy with the corner's parity holds it brick-aligned: brick (X + (X & 1)) >> 1
+                const int Z0 = iz - 1;
+                q.base = pack_corner(ix, iy, Z0);
+                q.c0 = (Z0 + (Z0 & 1)) >> 1; q.c1 = (iy + (iy & 1)) >> 1; q.c2 = (ix + (ix & 1)) >> 1;
+                q.c3 = ((ix & 1) << 2) | ((iy & 1) << 1) | (Z0 & 1);
+            } else {
+                q.base = (unsigned)corner_zfast(g, ix, iy, iz);        // same validity flag and offsets as the LDG kernels
+                q.c0 = 4 * (iz - 1); q.c1 = iy; q.c2 = ix;             // stored index s holds node s - 1: the stencil corner (ix-1, iy-1) is stored at (ix, iy)
+            }
         } else q.tz = 0.f;
         q.cf = coef[p];
     }
     return q;
 }
 
+template <bool BRICKS>
 __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_constant__ CUtensorMap tmap, GridGeom g, long long n, const float* __restrict__ pos,
                                                              const float4* __restrict__ coef, float* __restrict__ E, float* __restrict__ F,
                                                              const unsigned* __restrict__ choice) {
@@ -92,18 +108,27 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
         const unsigned mine = (valid >> (16 * hb)) & 0xFFFFu;
         if (lane == 0) mbar_expect_tx(bar + hb, 1024u * (unsigned)__popc(mine));
         __syncwarp();
-        if (half == hb && q.base != kNoStencil) tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
+        if (half == hb && q.base != kNoStencil) {
+            if (BRICKS) tma_box5(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, q.c3, bar + hb);
+            else tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
+        }
     };
+    // raw box -> tile element: z-fastest rows land in tile order (node lane = 4 row + k); a brick box lands as [bx][by][bz][dx dy dz]: float4 lane of
+    // the first half is node a = dx, b = 2 by + dy, k = 2 bz + dz (the second half: a + 2)
+    const int e0 = BRICKS ? (((lane >> 2) & 1) << 4) | (((((lane >> 4) & 1) << 1) | ((lane >> 1) & 1)) << 2) | ((((lane >> 3) & 1) << 1) | (lane & 1)) : lane;
     // A tile whose points share stencil lines (spatially sorted input: warp_points_are_local) is gathered through the L1 instead, as k_eval_coop
     // does: L1 / L2 hits are worth more than the TMA's independence from the LSU.  Its buffers are simply not armed.
-    auto is_clustered = [&](const Pt& q) { return warp_points_are_local(q.c2, q.c1, q.c0 >> 2, q.base != kNoStencil, lane); };
-    Pt cur = load_point(g, t * 32 + lane, n, pos, coef);
+    auto is_clustered = [&](const Pt& q) {
+        if (BRICKS) return warp_points_are_local((int)(q.base & 2047u), (int)((q.base >> kCornerBits) & 2047u), (int)(q.base >> (2 * kCornerBits)), q.base != kNoStencil, lane);
+        return warp_points_are_local(q.c2, q.c1, q.c0 >> 2, q.base != kNoStencil, lane);
+    };
+    Pt cur = load_point<BRICKS>(g, t * 32 + lane, n, pos, coef);
     bool cur_cl = is_clustered(cur);
     if (t < n_tiles && !cur_cl) { issue(cur, 0); issue(cur, 1); }
     unsigned parity = 0;
     for (; t < n_tiles; t += stride) {
         const long long tn = t + stride;
-        Pt nxt = load_point(g, tn < n_tiles ? tn * 32 + lane : n, n, pos, coef);       // p = n: an empty point
+        Pt nxt = load_point<BRICKS>(g, tn < n_tiles ? tn * 32 + lane : n, n, pos, coef);       // p = n: an empty point
         const bool nxt_cl = is_clustered(nxt);
         s_cf[lane] = cur.cf; s_base[lane] = cur.base;
         __syncwarp();
@@ -111,7 +136,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
 #pragma unroll 8
             for (int q = 0; q < 32; ++q) {
                 const unsigned b = s_base[q];
-                if (b != kNoStencil) gather_rows<false>(g, b, s_cf[q], lane, q, tile);
+                if (b != kNoStencil) { if (BRICKS) gather_bricks<false>(g, b, s_cf[q], lane, q, tile); else gather_rows<false>(g, b, s_cf[q], lane, q, tile); }
             }
             if (tn < n_tiles && !nxt_cl) { issue(nxt, 0); issue(nxt, 1); }
         } else {
@@ -122,7 +147,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
 #pragma unroll 4
                 for (int q = 0; q < 16; ++q) {
                     if (s_base[16 * hb + q] != kNoStencil)
-                        store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], lane, 16 * hb + q, tile);
+                        store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], e0, 16 * hb + q, tile);
                 }
                 __syncwarp();                              // every lane has read this half: the buffer can take the next tile's boxes
                 if (tn < n_tiles && !nxt_cl) issue(nxt, hb);
@@ -153,6 +178,7 @@ namespace gridff {
 // Encode the ZFAST store as a 3-D tensor of fp32 {nzp * 4, sy, sx} with a {16, 4, 4} box (driver entry point looked up at run time: the
 // library does not link libcuda).  Returns 0 and fills grid->tmap on success.
 int make_tensor_map(gridff_grid* grid) {
+    grid->tmap_ok = 0;
     static EncodeTiledFn encode = nullptr;
     if (!encode) {
         void* fn = nullptr; cudaDriverEntryPointQueryResult qr;
@@ -162,6 +188,19 @@ int make_tensor_map(gridff_grid* grid) {
     }
     const GridGeom& G = grid->geom;
     static_assert(sizeof(CUtensorMap) <= sizeof(grid->tmap), "tensor map storage");
+    if (G.n_copies == 8) {
+        // 8-copy micro-brick store: fp32 {32 (a brick), nbz, nby, nbx, 8 copies}, box {32, 2, 2, 2, 1} = the 8 bricks of a stencil in its aligned copy
+        const cuuint64_t dims[5] = {32, (cuuint64_t)G.nbz, (cuuint64_t)G.nby, (cuuint64_t)G.nbx, 8};
+        const cuuint64_t strides[4] = {128, (cuuint64_t)G.nbz * 128, (cuuint64_t)G.nby * G.nbz * 128, (cuuint64_t)G.copy_stride * 16};
+        const cuuint32_t box[5] = {32, 2, 2, 2, 1}, estr[5] = {1, 1, 1, 1, 1};
+        CUtensorMap m;
+        CUresult r = encode(&m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 5, (void*)G.store, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                            CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled (bricks) failed (%d)", (int)r); return GRIDFF_ECUDA; }
+        memcpy(grid->tmap, &m, sizeof(m));
+        grid->tmap_ok = 1;
+        return GRIDFF_OK;
+    }
     const cuuint64_t dims[3] = {(cuuint64_t)G.nzp * 4, (cuuint64_t)G.sy, (cuuint64_t)G.sx};
     const cuuint64_t strides[2] = {(cuuint64_t)G.nzp * 16, (cuuint64_t)G.sy * G.nzp * 16};         // bytes, dims 1 and 2
     const cuuint32_t box[3] = {16, 4, 4}, estr[3] = {1, 1, 1};
@@ -183,21 +222,23 @@ int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const flo
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     const size_t smem = kTmaWarps * ((kWarpSmem + 1023) & ~(size_t)1023) + 128;
-    static bool attr_set = false;
-    if (!attr_set) {
-        GRIDFF_CUDA(cudaFuncSetAttribute(k_eval_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        GRIDFF_CUDA(cudaFuncSetAttribute(k_eval_tma, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        attr_set = true;
+    const bool bricks = grid->geom.n_copies == 8;
+    auto kern = bricks ? k_eval_tma<true> : k_eval_tma<false>;
+    static bool attr_set[2] = {false, false};
+    if (!attr_set[bricks]) {
+        GRIDFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        GRIDFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        attr_set[bricks] = true;
     }
     int per_sm = 1;
-    GRIDFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_eval_tma, kTmaWarps * 32, smem));
+    GRIDFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTmaWarps * 32, smem));
     if (per_sm < 1) per_sm = 1;
     const long long n_tiles = (n + 31) / 32;
     long long blocks = (long long)sms * per_sm;
     if (blocks * kTmaWarps > n_tiles) blocks = (n_tiles + kTmaWarps - 1) / kTmaWarps;
     CUtensorMap m;
     memcpy(&m, grid->tmap, sizeof(m));
-    cudaError_t e = launch_with_window(grid, k_eval_tma, dim3((unsigned)blocks), dim3(kTmaWarps * 32), smem, st, m, grid->geom, n, d_pos, (const float4*)d_coef, d_E, d_F, d_choice);
+    cudaError_t e = launch_with_window(grid, kern, dim3((unsigned)blocks), dim3(kTmaWarps * 32), smem, st, m, grid->geom, n, d_pos, (const float4*)d_coef, d_E, d_F, d_choice);
     count_launch();
     if (e != cudaSuccess) return cuda_fail(e, "gridff_eval (TMA) launch");
     return GRIDFF_OK;

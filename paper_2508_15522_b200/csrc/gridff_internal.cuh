@@ -28,6 +28,9 @@ struct GridGeom {
     float inv_hx, inv_hy, inv_hz;
     float fnx, inv_nx, fny, inv_ny;   // (float)nx, 1/nx, ...: cell wrap without an integer division
     const float4* store;
+    // micro-brick stores (GRIDFF_LAYOUT_MBRICK*, gridff_derive.cu): bricks per axis and nodes per copy; 0 otherwise
+    int nbx, nby, nbz, n_copies;
+    long long copy_stride;
 };
 
 struct MolDev;   // packed molecule in device memory (gridff_replica.cu)
@@ -37,7 +40,8 @@ void set_error(const char* fmt, ...);
 int eval_derived(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);   // gridff_derive.cu
 constexpr unsigned kChoiceCoop = 1u, kChoiceTma = 2u;     // device-side kernel choice of gridff_eval (gridff_eval.cu: k_eval_classify)
 int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, const unsigned* d_choice, cudaStream_t st);       // gridff_eval_tma.cu
-int make_tensor_map(gridff_grid* grid);               // gridff_eval_tma.cu: CUtensorMap of a z-fastest fp32 store (0 on success)
+int make_tensor_map(gridff_grid* grid);               // gridff_eval_tma.cu: CUtensorMap of a z-fastest fp32 store or of an 8-copy micro-brick store (0 on success)
+int eval_bricks(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, int variant, cudaStream_t st);   // gridff_derive.cu
 int cuda_fail(cudaError_t e, const char* what);
 void count_launch(int n = 1);
 

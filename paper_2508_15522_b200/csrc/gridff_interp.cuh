@@ -133,7 +133,37 @@ __device__ __forceinline__ void load_rows(const GridGeom& g, unsigned base, int 
     const float4* p = g.store + base + (r0 >> 2) * ps + (r0 & 3) * rs + k;
     n0 = __ldg(p); n1 = __ldg(p + 2 * ps);
 }
-__device__ __forceinline__ void store_rows(const float4 cf, const float4 n0, const float4 n1, int lane, int slot, float* tile) {
+// e0: the tile element (4 row + k, 0..31) of n0; n1 is element e0 + 32
+__device__ __forceinline__ void store_rows(const float4 cf, const float4 n0, const float4 n1, int e0, int slot, float* tile) {
+    tile[tile_word(slot, e0)] = fold4(cf, n0);
+    tile[tile_word(slot, e0 + 32)] = fold4(cf, n1);
+}
+
+// ---- micro-brick stores (GRIDFF_LAYOUT_MBRICK / MBRICK2 / MBRICK8; built by gridff_grid_derive) ------------------------------------------
+// The parent's stored nodes (X, Y, Z) in 2 x 2 x 2-node bricks of 128 B, bricks in [x][y][z] order, 1, 2 or 8 copies.  Copy c has shift bits
+// (s_x, s_y, s_z): along an axis with s = 1 its bricks are anchored one node earlier, brick b covering {2b - 1, 2b}; stored index X sits in brick
+// (X + s) >> 1 at position (X + s) & 1.  A stencil whose corner is odd along an axis is brick-aligned in a copy shifted along that axis.
+constexpr int kCornerBits = 11;                            // packed corner: X | Y << 11 | Z << 22  (sx, sy <= 2047, nzp <= 1023)
+__device__ __forceinline__ unsigned pack_corner(int X, int Y, int Z) { return (unsigned)X | ((unsigned)Y << kCornerBits) | ((unsigned)Z << (2 * kCornerBits)); }
+__host__ __device__ __forceinline__ int brick_shift_bits(int n_copies, int copy) { return n_copies == 8 ? copy : (n_copies == 2 && copy) ? 7 : 0; }
+// the copy in which the stencil with corner (X0, Y0, Z0) touches the fewest bricks
+__device__ __forceinline__ int brick_copy(int n_copies, int X0, int Y0, int Z0) {
+    const int par = ((X0 & 1) << 2) | ((Y0 & 1) << 1) | (Z0 & 1);
+    return n_copies == 8 ? par : n_copies == 2 ? (__popc(par) >= 2 ? 1 : 0) : 0;
+}
+__device__ __forceinline__ size_t brick_node(const GridGeom& g, int copy, int sh, int X, int Y, int Z) {
+    X += (sh >> 2) & 1; Y += (sh >> 1) & 1; Z += sh & 1;
+    return (size_t)copy * (size_t)g.copy_stride + ((((size_t)(X >> 1) * g.nby + (Y >> 1)) * g.nbz + (Z >> 1)) << 3) + (size_t)(((X & 1) << 2) | ((Y & 1) << 1) | (Z & 1));
+}
+// warp-cooperative gather of one stencil from a micro-brick store: lane <-> node (a, b, k) as in gather_rows, so the tile is the same
+template <bool L2_ONLY>
+__device__ __forceinline__ void gather_bricks(const GridGeom& g, unsigned corner, const float4 cf, int lane, int slot, float* tile) {
+    const int X0 = (int)(corner & 2047u), Y0 = (int)((corner >> kCornerBits) & 2047u), Z0 = (int)(corner >> (2 * kCornerBits));
+    const int copy = brick_copy(g.n_copies, X0, Y0, Z0), sh = brick_shift_bits(g.n_copies, copy);
+    const int k = lane & 3, r0 = lane >> 2;
+    const float4* p = g.store + brick_node(g, copy, sh, X0 + (r0 >> 2), Y0 + (r0 & 3), Z0 + k);
+    const size_t plane = (size_t)g.nby * g.nbz * 8;        // a + 2: the next brick along x
+    const float4 n0 = L2_ONLY ? __ldcg(p) : __ldg(p), n1 = L2_ONLY ? __ldcg(p + plane) : __ldg(p + plane);
     tile[tile_word(slot, lane)] = fold4(cf, n0);
     tile[tile_word(slot, lane + 32)] = fold4(cf, n1);
 }

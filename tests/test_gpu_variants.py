@@ -69,6 +69,62 @@ def test_trilinear_foil_parity(api, orc, cfg1s):
     assert np.abs(E[sel] - Es[sel]).max() > 1e-4
 
 
+@pytest.mark.parametrize("k", [1, 3])
+def test_micro_brick_stores_match_zfast_and_oracle(api, orc, cfg1s, cfg3s, k):
+    """GRIDFF_LAYOUT_MBRICK / MBRICK2 / MBRICK8 (the fp32 coefficients in 2x2x2-node bricks of one 128-byte line, 1 / 2 / 8 shifted copies;
+    the layout for stores beyond the L2, "limited by global memory access"): gridff_eval returns the z-fastest store's
+    numbers BIT FOR BIT (LDG gather, and the 5-D TMA box kernel of the 8-copy store), on random points with every corner parity, cell
+    faces, periodic wraps, the lowest and the highest cell, points below node 1 and above the domain, for several point counts (one point,
+    a ragged tail, many tiles per persistent warp); and those numbers are the oracle's within north_star's tolerances."""
+    cfg = cfg1s if k == 1 else cfg3s
+    d = cfg["desc"]
+    g = gpu_grid(api, cfg["sub"], d)
+    nx, ny, nz = inputs.grid_dims(d)
+    z0 = d["z_ref"] + d["z_lo"]; hx, hy, hz = d["Lx"] / nx, d["Ly"] / ny, d["spacing"]
+    stores = [(lay, api.gridff_grid_derive(g, lay)) for lay in (api.LAYOUT_MBRICK, api.LAYOUT_MBRICK2, api.LAYOUT_MBRICK8)]
+    for n in (1, 31, 33, 5000, 150011):
+        pos, coef = eval_points(cfg, n, 300 + n)
+        if n >= 5000:
+            # every cell along the x and y edges (the 3-node halo of the store), the lowest cells (1) and the highest (nz - 3), both parities
+            m = 1024
+            ii = np.arange(m)
+            pos[:m, 0] = ((ii % 8) - 4 + 0.37) * hx; pos[:m, 1] = (((ii // 8) % 8) - 4 + 0.61) * hy
+            pos[:m, 2] = z0 + np.where(ii % 2 == 0, 1.0 + (ii // 64) % 3, nz - 3 - (ii // 64) % 3 + 0.999) * hz
+            pos[m:m + 8] = [[0.0, 0.0, z0 + 2 * hz], [d["Lx"], d["Ly"], z0 + 3 * hz], [-1e-7, d["Ly"], z0 + 4 * hz], [hx, hy, z0 + hz],
+                            [d["Lx"] - 1e-6, 0.5 * hy, z0 + 0.5 * hz], [3.5 * hx, -1e-6, z0 + (nz - 2) * hz - 1e-4],
+                            [0.5 * hx, 0.5 * hy, z0 + (nz - 2) * hz + 1e-3], [7 * d["Lx"] + 0.3, -5 * d["Ly"] - 0.2, z0 + 5.5 * hz]]
+        dp, dc = dev(pos), dev(coef)
+        E2, F2 = api.gridff_eval(g, dp, dc, variant=2)
+        for lay, gb in stores:
+            for variant in ((0, 2, 3) if lay == api.LAYOUT_MBRICK8 else (0, 2)):
+                Eb, Fb = api.gridff_eval(gb, dp, dc, variant=variant)
+                assert bool(torch.equal(E2, Eb)) and bool(torch.equal(F2, Fb)), (lay, variant, n)
+    og, _ = oracle_grid(orc, cfg["sub"], d)
+    Eo, Fo, Vc, _ = orc.interp(og, pos, coef, channels=True)
+    den = np.sum(np.abs(coef[:, :3].astype(np.float64) * Vc), axis=1)
+    ok = den > 1e-12
+    Eg, Fg = Eb.cpu().numpy().astype(np.float64), Fb.cpu().numpy().astype(np.float64)
+    assert (np.abs(Eg - Eo)[ok] / den[ok]).max() <= 1e-5 and np.abs(Fg - Fo).max() <= 1e-4
+    above = (pos[:, 2].astype(np.float64) - z0) / hz >= nz - 2
+    assert above.sum() > 0 and np.all(Eg[above] == 0) and np.all(Fg[above] == 0)
+    # E or F alone, the 8-copy store's TMA kernel
+    E3, none = api.gridff_eval(stores[2][1], dp, dc, variant=3, want_F=False)
+    none2, F3 = api.gridff_eval(stores[2][1], dp, dc, variant=3, want_E=False)
+    assert none is None and none2 is None and bool(torch.equal(E3, E2)) and bool(torch.equal(F3, F2))
+    # sizes: 1 / 2 / 8 copies of (sx/2 + 1)(sy/2 + 1)(nzp/2 + 1) bricks of 128 B; misuse is refused
+    nzp = (nz + 7) // 8 * 8
+    per_copy = ((nx + 3) // 2 + 1) * ((ny + 3) // 2 + 1) * (nzp // 2 + 1) * 128
+    assert [gb.store.numel() for _, gb in stores] == [per_copy, 2 * per_copy, 8 * per_copy]
+    with pytest.raises(api.GridffError):
+        api.gridff_eval(stores[0][1], dp, dc, variant=3)          # TMA needs the 8-copy store
+    with pytest.raises(api.GridffError):
+        api.gridff_eval(stores[2][1], dp, dc, variant=1)
+    with pytest.raises(api.GridffError):
+        api.gridff_grid_derive(stores[2][1], api.LAYOUT_HALF)     # derived from derived
+    with pytest.raises(api.GridffError):
+        api.gridff_grid_export(stores[2][1])
+
+
 def test_derive_errors(api, cfg1s):
     g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
     gb = gpu_grid(api, cfg1s["sub"], cfg1s["desc"], layout=1)
