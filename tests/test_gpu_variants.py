@@ -8,8 +8,8 @@ import pytest
 import torch
 
 from paper_2508_15522_b200 import inputs
-from gridff_cases import oracle_grid, gpu_grid, small_config
-from test_gpu_parity import api, dev, cfg1s, eval_points  # noqa: F401
+from gridff_cases import oracle_grid, gpu_grid, small_config, energy_denominator
+from test_gpu_parity import api, dev, cfg1s, cfg3s, eval_points  # noqa: F401
 
 pytestmark = pytest.mark.gpu
 
@@ -101,7 +101,7 @@ def test_micro_brick_stores_match_zfast_and_oracle(api, orc, cfg1s, cfg3s, k):
                 assert bool(torch.equal(E2, Eb)) and bool(torch.equal(F2, Fb)), (lay, variant, n)
     og, _ = oracle_grid(orc, cfg["sub"], d)
     Eo, Fo, Vc, _ = orc.interp(og, pos, coef, channels=True)
-    den = np.sum(np.abs(coef[:, :3].astype(np.float64) * Vc), axis=1)
+    den = energy_denominator(coef.astype(np.float64), Vc)
     ok = den > 1e-12
     Eg, Fg = Eb.cpu().numpy().astype(np.float64), Fb.cpu().numpy().astype(np.float64)
     assert (np.abs(Eg - Eo)[ok] / den[ok]).max() <= 1e-5 and np.abs(Fg - Fo).max() <= 1e-4
