@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_eval_half(GridGeom g, long long
     float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
     if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2]); cf = coef[p]; }
     s_base[w][lane] = s.base; s_cf[w][lane] = cf;
-    __syncwarp();
+    warp_sync();
     float* tile = s_tile[w];
     const uint2* store = reinterpret_cast<const uint2*>(g.store);
     const int k = lane & 3, r0 = lane >> 2;
@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_eval_half(GridGeom g, long long
             tile[tile_word(q, lane + 32)] = fold_half(c, n1);
         }
     }
-    __syncwarp();
+    warp_sync();
     if (p >= n) return;
     float e, fx, fy, fz;
     interp_tile(g, s, lane, tile, e, fx, fy, fz);
@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_eval_bricks(GridGeom g, long lo
     if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz); cf = coef[p]; }
     s_corner[w][lane] = s.base == kNoStencil ? kNoStencil : pack_corner(ix, iy, iz - 1);
     s_cf[w][lane] = cf;
-    __syncwarp();
+    warp_sync();
     float* tile = s_tile[w];
     if (warp_points_are_local(ix, iy, iz, s.base != kNoStencil, lane)) {
 #pragma unroll 8
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kWarps * 32) k_eval_bricks(GridGeom g, long lo
             if (c != kNoStencil) gather_bricks<true>(g, c, s_cf[w][q], lane, q, tile);
         }
     }
-    __syncwarp();
+    warp_sync();
     if (p >= n) return;
     float e, fx, fy, fz;
     interp_tile(g, s, lane, tile, e, fx, fy, fz);

@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
     int ix = 0, iy = 0, iz = 0;
     if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz); cf = coef[p]; }
     s_base[w][lane] = s.base; s_cf[w][lane] = cf;
-    __syncwarp();
+    warp_sync();
     float* tile = s_tile[w];
     // do this warp's points share stencil lines?  (spatially sorted input)  Then the L1 pays; otherwise gather past it
     const bool clustered = warp_points_are_local(ix, iy, iz, s.base != kNoStencil, lane);
@@ -55,7 +55,7 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
             if (b != kNoStencil) gather_rows<true>(g, b, s_cf[w][q], lane, q, tile);
         }
     }
-    __syncwarp();
+    warp_sync();
     if (p >= n) return;
     float e, fx, fy, fz;
     interp_tile(g, s, lane, tile, e, fx, fy, fz);

@@ -97,7 +97,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_base + 32);
     if (lane == 0) { mbar_init(bar, 1); mbar_init(bar + 1, 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncwarp();
+    warp_sync();
 
     const long long n_tiles = (n + 31) / 32, stride = (long long)gridDim.x * kTmaWarps;
     long long t = (long long)blockIdx.x * kTmaWarps + w;
@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
         const unsigned valid = __ballot_sync(0xFFFFFFFFu, q.base != kNoStencil);
         const unsigned mine = (valid >> (16 * hb)) & 0xFFFFu;
         if (lane == 0) mbar_expect_tx(bar + hb, 1024u * (unsigned)__popc(mine));
-        __syncwarp();
+        warp_sync();
         if (half == hb && q.base != kNoStencil) {
             if (BRICKS) tma_box5(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, q.c3, bar + hb);
             else tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
@@ -131,7 +131,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
         Pt nxt = load_point<BRICKS>(g, tn < n_tiles ? tn * 32 + lane : n, n, pos, coef);       // p = n: an empty point
         const bool nxt_cl = is_clustered(nxt);
         s_cf[lane] = cur.cf; s_base[lane] = cur.base;
-        __syncwarp();
+        warp_sync();
         if (cur_cl) {
 #pragma unroll 8
             for (int q = 0; q < 32; ++q) {
@@ -143,18 +143,19 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
 #pragma unroll
             for (int hb = 0; hb < 2; ++hb) {
                 mbar_wait(bar + hb, parity);
+                stress_delay();
                 const float4* r4 = raw[hb];
 #pragma unroll 4
                 for (int q = 0; q < 16; ++q) {
                     if (s_base[16 * hb + q] != kNoStencil)
                         store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], e0, 16 * hb + q, tile);
                 }
-                __syncwarp();                              // every lane has read this half: the buffer can take the next tile's boxes
+                warp_sync();                              // every lane has read this half: the buffer can take the next tile's boxes
                 if (tn < n_tiles && !nxt_cl) issue(nxt, hb);
             }
             parity ^= 1;
         }
-        __syncwarp();
+        warp_sync();
         const long long p = t * 32 + lane;
         if (p < n) {
             Stencil s; s.base = cur.base; s.tx = cur.tx; s.ty = cur.ty; s.tz = cur.tz;
@@ -163,7 +164,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
             if (E) E[p] = e;
             if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
         }
-        __syncwarp();                                      // the folded tile and s_cf / s_base are rewritten in the next trip
+        warp_sync();                                      // the folded tile and s_cf / s_base are rewritten in the next trip
         cur = nxt; cur_cl = nxt_cl;
     }
 }

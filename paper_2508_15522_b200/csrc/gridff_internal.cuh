@@ -58,6 +58,28 @@ void count_launch(int n = 1);
         if (e__ != cudaSuccess) return gridff::cuda_fail(e__, name); \
     } while (0)
 
+// ---- race stress build (-DGRIDFF_STRESS; csrc/build.py build_stress, tests/test_gpu_stress.py) ------------------
+// compute-sanitizer's racecheck is not available on the GPU pool, so the hand-overs through shared memory are tested by perturbing the
+// schedule instead: in the stress build every synchronisation point is surrounded by a pseudo-random per-LANE delay (one lane in four sleeps
+// up to ~1 us, keyed on the clock, the lane and the warp), so that lanes and warps that normally run in lock-step reach the hand-overs at
+// very different times.  A missing or misplaced barrier then changes results; the test compares the stress build with the plain build bit
+// for bit.  In the product build stress_delay() is empty.
+#ifdef GRIDFF_STRESS
+__device__ __forceinline__ void stress_delay() {
+    unsigned c, l, w;
+    asm volatile("mov.u32 %0, %%clock;" : "=r"(c));
+    asm volatile("mov.u32 %0, %%laneid;" : "=r"(l));
+    asm volatile("mov.u32 %0, %%warpid;" : "=r"(w));
+    unsigned h = c ^ (l * 0x9E3779B9u) ^ (w * 0x85EBCA6Bu);
+    h ^= h >> 15; h *= 0x2C1B3C6Du; h ^= h >> 12; h *= 0x297A2D39u; h ^= h >> 15;
+    if ((h & 3u) == 0u) __nanosleep(h >> 22);
+}
+#else
+__device__ __forceinline__ void stress_delay() {}
+#endif
+// __syncwarp() with the stress delays around it
+__device__ __forceinline__ void warp_sync() { stress_delay(); __syncwarp(); stress_delay(); }
+
 // ---- B-spline weights (Eqs. 5-6; polynomial pieces of B(t+1-j), j = 0..3) -------------------
 __device__ __forceinline__ void bspline_w(float t, float w[4], float d[4]) {
     const float s = 1.0f - t, t2 = t * t, s2 = s * s;
