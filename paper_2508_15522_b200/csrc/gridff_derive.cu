@@ -148,7 +148,8 @@ __global__ void k_to_bricks(GridGeom parent, GridGeom g, float4* __restrict__ ds
 // k_eval_coop over bricks: a warp owns 32 points, gathers each stencil cooperatively (lane <-> node as over the z-fastest store, so the folded
 // tile, the contraction and the results are the same bit for bit), every lane then contracts its own point
 __global__ void __launch_bounds__(kWarps * 32) k_eval_bricks(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
-                                                             float* __restrict__ E, float* __restrict__ F) {
+                                                             float* __restrict__ E, float* __restrict__ F, const unsigned* __restrict__ choice) {
+    if (choice && *choice != kChoiceCoop) return;         // the device-side choice (k_eval_classify) went to the TMA kernel
     __shared__ __align__(16) float s_tile[kWarps][32 * 64];
     __shared__ __align__(16) float4 s_cf[kWarps][32];
     __shared__ unsigned s_corner[kWarps][32];
@@ -194,9 +195,18 @@ int eval_bricks(const gridff_grid* grid, long long n, const float* d_pos, const 
     const GridGeom& G = grid->geom;
     if (variant != 0 && variant != 2 && variant != 3) { set_error("micro-brick stores have variants 0, 2 (LDG gather) and 3 (TMA, 8 copies)"); return GRIDFF_EINVAL; }
     if (variant == 3 && !(G.n_copies == 8 && grid->tmap_ok)) { set_error("the TMA variant needs the 8-copy micro-brick store and a tensor map"); return GRIDFF_EUNSUPPORTED; }
-    if (variant == 3 || (variant == 0 && G.n_copies == 8 && grid->tmap_ok && n >= 4096)) return eval_tma(grid, n, d_pos, d_coef, d_E, d_F, nullptr, st);
+    if (variant == 3) return eval_tma(grid, n, d_pos, d_coef, d_E, d_F, nullptr, st);
+    // 8-copy store, default: scattered points go to the TMA box kernel, spatially sorted ones to the LDG gather (L1 / L2 hits at full occupancy);
+    // the order of the caller's points is classified on the device and both kernels are enqueued (gridff_eval.cu: k_eval_classify)
+    const unsigned* choice = nullptr;
+    if (variant == 0 && G.n_copies == 8 && grid->tmap_ok && n >= 4096) {
+        int rc = classify_points(grid, n, d_pos, st, &choice);
+        if (rc) return rc;
+        rc = eval_tma(grid, n, d_pos, d_coef, d_E, d_F, choice, st);
+        if (rc) return rc;
+    }
     const long long per_block = kWarps * 32;
-    cudaError_t e = launch_with_window(grid, k_eval_bricks, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F);
+    cudaError_t e = launch_with_window(grid, k_eval_bricks, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F, choice);
     count_launch();
     if (e != cudaSuccess) return cuda_fail(e, "gridff_eval (micro-brick store) launch");
     return GRIDFF_OK;

@@ -180,6 +180,22 @@ bool store_exceeds_l2(const gridff_grid* grid) {
 }  // namespace
 
 
+namespace gridff {
+
+// enqueue k_eval_classify; *choice = the device word it writes (kChoiceCoop: spatially sorted points, kChoiceTma: scattered)
+int classify_points(const gridff_grid* grid, long long n, const float* d_pos, cudaStream_t st, const unsigned** choice) {
+    static std::atomic<unsigned> next{0};
+    unsigned* words = nullptr;
+    GRIDFF_CUDA(cudaGetSymbolAddress((void**)&words, g_eval_choice));
+    unsigned* w = words + (next.fetch_add(1, std::memory_order_relaxed) & 63u);
+    k_eval_classify<<<1, 256, 0, st>>>(grid->geom, n, d_pos, w);
+    GRIDFF_LAUNCH_CHECK("k_eval_classify");
+    *choice = w;
+    return GRIDFF_OK;
+}
+
+}  // namespace gridff
+
 extern "C" {
 
 int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F,
@@ -203,20 +219,16 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
     } else if (variant == 0 || variant == 2) {
         // default for a store that does not fit the L2: classify the point order on the device, then launch both kernels (see k_eval_classify).
         // L2-resident stores: the LDG gather alone (1.4x the TMA kernel there).
-        unsigned* choice = nullptr;
+        const unsigned* choice = nullptr;
         if (variant == 0 && grid->tmap_ok && n >= 4096 && store_exceeds_l2(grid)) {
-            static std::atomic<unsigned> next{0};
-            unsigned* words = nullptr;
-            GRIDFF_CUDA(cudaGetSymbolAddress((void**)&words, g_eval_choice));
-            choice = words + (next.fetch_add(1, std::memory_order_relaxed) & 63u);
-            k_eval_classify<<<1, 256, 0, st>>>(G, n, d_pos, choice);
-            GRIDFF_LAUNCH_CHECK("k_eval_classify");
-            int rc = eval_tma(grid, n, d_pos, d_coef, d_E, d_F, choice, st);
+            int rc = classify_points(grid, n, d_pos, st, &choice);
+            if (rc) return rc;
+            rc = eval_tma(grid, n, d_pos, d_coef, d_E, d_F, choice, st);
             if (rc) return rc;
         }
         const long long per_block = kEvalWarps * 32;
         e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F,
-                               (const unsigned*)choice);
+                               choice);
     } else { set_error("unknown eval variant %d", variant); return GRIDFF_EINVAL; }
     count_launch();
     if (e != cudaSuccess) return cuda_fail(e, "gridff_eval launch");

@@ -22,7 +22,9 @@ using namespace gridff;
 namespace {
 
 constexpr int kTmaWarps = 1;                       // warps per block: a warp is self-contained (own buffers, own barriers)
-constexpr int kRawHalf = 16 * 1024;                // 16 points x 1 KB
+constexpr int kGroupPts = 8;                       // points whose boxes share a raw buffer and an mbarrier: a tile of 32 points arrives in 32 / kGroupPts groups,
+constexpr int kGroups = 32 / kGroupPts;            // alternating between two buffers (kGroups even).  8 points: 24.6 KB per warp, 9 warps per SM (16: 41 KB, 5 warps)
+constexpr int kRawHalf = kGroupPts * 1024;         // one raw buffer
 constexpr size_t kWarpSmem = 2 * kRawHalf + 32 * 64 * 4 + 32 * 16 + 32 * 4 + 2 * 8;      // raw A, raw B, folded tile, cf, base, 2 mbarriers
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -101,16 +103,17 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
 
     const long long n_tiles = (n + 31) / 32, stride = (long long)gridDim.x * kTmaWarps;
     long long t = (long long)blockIdx.x * kTmaWarps + w;
-    const int half = lane >> 4;
-    // arm one half-buffer with the boxes of the points of `q` that sit in it (the lanes of that half own them)
-    auto issue = [&](const Pt& q, int hb) {
+    const int my_group = lane / kGroupPts;
+    // arm buffer (grp & 1) with the boxes of group `grp` of the points `q` (the lanes of that group own them)
+    auto issue = [&](const Pt& q, int grp) {
+        const int hb = grp & 1;
         const unsigned valid = __ballot_sync(0xFFFFFFFFu, q.base != kNoStencil);
-        const unsigned mine = (valid >> (16 * hb)) & 0xFFFFu;
+        const unsigned mine = (valid >> (kGroupPts * grp)) & ((1u << kGroupPts) - 1u);
         if (lane == 0) mbar_expect_tx(bar + hb, 1024u * (unsigned)__popc(mine));
         warp_sync();
-        if (half == hb && q.base != kNoStencil) {
-            if (BRICKS) tma_box5(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, q.c3, bar + hb);
-            else tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & 15) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
+        if (my_group == grp && q.base != kNoStencil) {
+            if (BRICKS) tma_box5(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & (kGroupPts - 1)) * 1024, &tmap, q.c0, q.c1, q.c2, q.c3, bar + hb);
+            else tma_box(reinterpret_cast<unsigned char*>(raw[hb]) + (lane & (kGroupPts - 1)) * 1024, &tmap, q.c0, q.c1, q.c2, bar + hb);
         }
     };
     // raw box -> tile element: z-fastest rows land in tile order (node lane = 4 row + k); a brick box lands as [bx][by][bz][dx dy dz]: float4 lane of
@@ -125,7 +128,7 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
     Pt cur = load_point<BRICKS>(g, t * 32 + lane, n, pos, coef);
     bool cur_cl = is_clustered(cur);
     if (t < n_tiles && !cur_cl) { issue(cur, 0); issue(cur, 1); }
-    unsigned parity = 0;
+    unsigned parity[2] = {0u, 0u};
     for (; t < n_tiles; t += stride) {
         const long long tn = t + stride;
         Pt nxt = load_point<BRICKS>(g, tn < n_tiles ? tn * 32 + lane : n, n, pos, coef);       // p = n: an empty point
@@ -141,19 +144,21 @@ __global__ void __launch_bounds__(kTmaWarps * 32) k_eval_tma(const __grid_consta
             if (tn < n_tiles && !nxt_cl) { issue(nxt, 0); issue(nxt, 1); }
         } else {
 #pragma unroll
-            for (int hb = 0; hb < 2; ++hb) {
-                mbar_wait(bar + hb, parity);
+            for (int grp = 0; grp < kGroups; ++grp) {
+                const int hb = grp & 1;
+                mbar_wait(bar + hb, parity[hb]);
+                parity[hb] ^= 1u;
                 stress_delay();
                 const float4* r4 = raw[hb];
 #pragma unroll 4
-                for (int q = 0; q < 16; ++q) {
-                    if (s_base[16 * hb + q] != kNoStencil)
-                        store_rows(s_cf[16 * hb + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], e0, 16 * hb + q, tile);
+                for (int q = 0; q < kGroupPts; ++q) {
+                    if (s_base[kGroupPts * grp + q] != kNoStencil)
+                        store_rows(s_cf[kGroupPts * grp + q], r4[q * 64 + lane], r4[q * 64 + 32 + lane], e0, kGroupPts * grp + q, tile);
                 }
-                warp_sync();                              // every lane has read this half: the buffer can take the next tile's boxes
-                if (tn < n_tiles && !nxt_cl) issue(nxt, hb);
+                warp_sync();                              // every lane has read this buffer: it can take the boxes of the group after next
+                if (grp + 2 < kGroups) issue(cur, grp + 2);
+                else if (tn < n_tiles && !nxt_cl) issue(nxt, grp + 2 - kGroups);
             }
-            parity ^= 1;
         }
         warp_sync();
         const long long p = t * 32 + lane;

@@ -68,22 +68,22 @@ __global__ void __launch_bounds__(1024) k_filter_append(const FilterParams P) {
         ++n_cand;
         if (f > 0) continue;
         if (threadIdx.x == 0) s_hit = 0;
-        stress_delay(); __syncthreads(); stress_delay();
+        stress_before_barrier(); __syncthreads(); stress_delay();
         const float Ec = P.E[r];
         const float* xc = P.pos + (size_t)r * 3 * P.n;
         bool m = false;
         for (int j = n0 + threadIdx.x; j < n_cur; j += blockDim.x) m = m || same_structure(P, Ec, xc, P.lib + (size_t)j * stride);
         if (m) s_hit = 1;
-        stress_delay(); __syncthreads(); stress_delay();
+        stress_before_barrier(); __syncthreads(); stress_delay();
         const bool hit = s_hit != 0;
-        stress_delay(); __syncthreads(); stress_delay();
+        stress_before_barrier(); __syncthreads(); stress_delay();
         if (hit) continue;
         if (n_cur >= P.cap) { ++n_drop; continue; }
         float* rec = P.lib + (size_t)n_cur * stride;
         if (threadIdx.x == 0) { rec[0] = (float)r; rec[1] = (float)P.tag; rec[2] = P.steps ? (float)P.steps[r] : 0.f; rec[3] = Ec; }
         for (int i = threadIdx.x; i < 3 * P.n; i += blockDim.x) rec[4 + i] = xc[i];
         ++n_cur; ++n_new;
-        stress_delay(); __syncthreads(); stress_delay();                              // the record is visible to the block before the next survivor is compared
+        stress_before_barrier(); __syncthreads(); stress_delay();                              // the record is visible to the block before the next survivor is compared
     }
     if (threadIdx.x == 0) {
         *P.n_lib = n_cur;

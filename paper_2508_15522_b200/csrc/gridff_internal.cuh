@@ -40,6 +40,7 @@ void set_error(const char* fmt, ...);
 int eval_derived(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, cudaStream_t st);   // gridff_derive.cu
 constexpr unsigned kChoiceCoop = 1u, kChoiceTma = 2u;     // device-side kernel choice of gridff_eval (gridff_eval.cu: k_eval_classify)
 int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, const unsigned* d_choice, cudaStream_t st);       // gridff_eval_tma.cu
+int classify_points(const gridff_grid* grid, long long n, const float* d_pos, cudaStream_t st, const unsigned** choice);       // gridff_eval.cu: device-side choice word
 int make_tensor_map(gridff_grid* grid);               // gridff_eval_tma.cu: CUtensorMap of a z-fastest fp32 store or of an 8-copy micro-brick store (0 on success)
 int eval_bricks(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, int variant, cudaStream_t st);   // gridff_derive.cu
 int cuda_fail(cudaError_t e, const char* what);
@@ -79,6 +80,12 @@ __device__ __forceinline__ void stress_delay() {}
 #endif
 // __syncwarp() with the stress delays around it
 __device__ __forceinline__ void warp_sync() { stress_delay(); __syncwarp(); stress_delay(); }
+// before an ALIGNED barrier (bar.sync, __syncthreads: every lane of a warp must arrive together): delay, then re-converge the warp
+__device__ __forceinline__ void stress_before_barrier() {
+#ifdef GRIDFF_STRESS
+    stress_delay(); __syncwarp();
+#endif
+}
 
 // ---- B-spline weights (Eqs. 5-6; polynomial pieces of B(t+1-j), j = 0..3) -------------------
 __device__ __forceinline__ void bspline_w(float t, float w[4], float d[4]) {
