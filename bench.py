@@ -382,9 +382,9 @@ def run_gridff(args, emit=True):
     probe = torch.empty(min(max(sb, 16 << 20), 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)
     l2 = {}
     for mode, key in ((0, "stream"), (1, "rows64")):
-        api.gridff_probe_read(probe, iters=20, mode=mode); torch.cuda.synchronize()
+        api.gridff_probe_read(probe, iters=100, mode=mode); torch.cuda.synchronize()        # warm: clocks up, buffer in L2
         best = 0.0
-        for _ in range(5):
+        for _ in range(10):
             a, b = ev(), ev()
             a.record(stream); api.gridff_probe_read(probe, iters=100, mode=mode); b.record(stream); b.synchronize()
             best = max(best, probe.numel() * 100 / (a.elapsed_time(b) * 1e-3) / 1e9)
@@ -577,9 +577,9 @@ def run_eval(args, emit=True):
         probe = torch.empty(min(max(nbytes, 16 << 20), 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)     # >= 16 MB: a smaller buffer cannot occupy every SM
         out = {}
         for mode, key in ((0, "stream"), (1, "rows64")):
-            api.gridff_probe_read(probe, iters=20, mode=mode); torch.cuda.synchronize()
+            api.gridff_probe_read(probe, iters=100, mode=mode); torch.cuda.synchronize()    # warm: clocks up, buffer in L2
             best = 0.0
-            for _ in range(5):
+            for _ in range(10):
                 a, b = ev(), ev()
                 a.record(stream); api.gridff_probe_read(probe, iters=100, mode=mode); b.record(stream); b.synchronize()
                 best = max(best, probe.numel() * 100 / (a.elapsed_time(b) * 1e-3) / 1e9)
