@@ -23,7 +23,7 @@ namespace {
 
 constexpr int kTmaWarps = 1;                       // warps per block: a warp is self-contained (own buffers, own barriers)
 constexpr int kGroupPts = 8;                       // points whose boxes share a raw buffer and an mbarrier: a tile of 32 points arrives in 32 / kGroupPts groups,
-constexpr int kGroups = 32 / kGroupPts;            // alternating between two buffers (kGroups even).  8 points: 24.6 KB per warp, 9 warps per SM (16: 41 KB, 5 warps)
+constexpr int kGroups = 32 / kGroupPts;            // alternating between two buffers (kGroups even).  8 points: 24.6 KB per warp, 8 warps per SM (16: 41 KB, 5 warps)
 constexpr int kRawHalf = kGroupPts * 1024;         // one raw buffer
 constexpr size_t kWarpSmem = 2 * kRawHalf + 32 * 64 * 4 + 32 * 16 + 32 * 4 + 2 * 8;      // raw A, raw B, folded tile, cf, base, 2 mbarriers
 
