@@ -5,6 +5,8 @@
     compute-sanitizer --tool synccheck python tests/sanitize_kernels.py
     compute-sanitizer --tool initcheck python tests/sanitize_kernels.py
 
+(On this GPU pool compute-sanitizer is closed — profiles/r2_sanitizers.md — so the script serves as the plain every-mode smoke run; the race
+evidence is tests/test_gpu_stress.py.)
 No oracle, no assertions on values (the parity tests do that): the point is that each code path runs under the tool, at sizes that keep
 the 100-1000x slow-down of racecheck within minutes.  Modes reached (printed as they run):
   grid build        Morse per-node and tiled sampling (magnitude window on / off), Coulomb, prefilters, z-fastest and 4x4x4-brick stores,

@@ -15,28 +15,46 @@ pytestmark = pytest.mark.gpu
 
 
 def test_half_store_parity(api, orc, cfg1s):
+    """fp16 coefficient store against the ORACLE's own half grid (fp64 -> fp32 -> fp16 of the oracle's coefficients; nothing taken from the GPU).
+    The GPU rounds ITS fp32 coefficients, which agree with the oracle's to half an fp32 ulp, so a coefficient that sits within one fp32 ulp of an
+    fp16 rounding boundary can land on the other side (about 2 in 10^4 nodes).  That effect is bounded from the oracle alone: D = the largest change
+    of a node's fp16 value when its fp32 value moves by one ulp (zero for all other nodes); with B-spline weights >= 0 and summing to 1, a point's
+    energy can move by at most sum_c |coef_c| max_stencil D_c and its force by 1.5 / h times that.  Asserted: north_star's tolerances plus that
+    bound, point by point — i.e. the plain 1e-5 / 1e-4 for the (majority of) points with no such node near their stencil."""
+    from scipy.ndimage import maximum_filter
     og, _ = oracle_grid(orc, cfg1s["sub"], cfg1s["desc"])
     g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
     gh = api.gridff_grid_derive(g, api.LAYOUT_HALF)
-    # the oracle rounds the GPU's own fp32 coefficients?  No: its own fp64 -> fp32 -> fp16.  The two fp32 stores agree to ~1e-7 relative,
-    # so a coefficient can land on the other side of an fp16 rounding boundary (1 in ~10^4): compare on the oracle's rounding of the
-    # exported GPU coefficients for the bit-level check, and on its own for the end-to-end one.
-    coef32 = api.gridff_grid_export(g).cpu().numpy()
-    hg_same = orc.OracleGrid(coef32.astype(np.float16).astype(np.float64), og.Lx, og.Ly, og.z0, og.hz)
     pos, cf = eval_points(cfg1s, 20011, 5)                        # ragged tail, many blocks
     E, F = api.gridff_eval(gh, dev(pos), dev(cf))
     E, F = E.cpu().numpy(), F.cpu().numpy()
-    Eo, Fo, Vc, _ = orc.interp(hg_same, pos, cf, channels=True)
+    hg = orc.half_grid(og)
+    Eh, Fh, Vc, _ = orc.interp(hg, pos, cf, channels=True)
     den = np.maximum(np.sum(np.abs(cf[:, :3].astype(np.float64) * Vc), axis=1), 1e-12)       # points above the domain: E = den = 0
-    assert (np.abs(E - Eo) / den).max() <= 1e-5
-    assert np.abs(F - Fo).max() <= 1e-4
-    # end to end against the oracle's own half grid: within the fp16 quantisation of a few boundary coefficients
-    Eh, Fh = orc.interp(orc.half_grid(og), pos, cf)
-    assert (np.abs(E - Eh) / den).max() <= 2e-3 and np.median(np.abs(E - Eh) / den) <= 1e-6
+    b32 = og.coef.astype(np.float32)
+    H = b32.astype(np.float16).astype(np.float64)
+    D = np.maximum(np.abs(np.nextafter(b32, np.float32(np.inf)).astype(np.float16).astype(np.float64) - H),
+                   np.abs(H - np.nextafter(b32, np.float32(-np.inf)).astype(np.float16).astype(np.float64)))
+    Dm = maximum_filter(D, size=(7, 7, 7, 1), mode=("wrap", "wrap", "nearest", "nearest"))      # covers the stencil and a cell of fp32 ambiguity
+    nx, ny, nz, nch = og.shape
+    hx, hy = og.Lx / nx, og.Ly / ny
+    ix = np.floor(pos[:, 0].astype(np.float64) / hx).astype(int) % nx
+    iy = np.floor(pos[:, 1].astype(np.float64) / hy).astype(int) % ny
+    iz = np.clip(np.floor((pos[:, 2].astype(np.float64) - og.z0) / og.hz).astype(int), 0, nz - 1)
+    slack = np.sum(np.abs(cf[:, :nch].astype(np.float64)) * Dm[ix, iy, iz], axis=1)
+    assert (slack == 0).mean() > 0.5, "the bound must leave most points at the plain tolerance"
+    assert np.all(np.abs(E - Eh) <= 1e-5 * den + slack), (np.abs(E - Eh) - slack).max()
+    assert np.all(np.abs(F - Fh).max(axis=1) <= 1e-4 + 1.5 / min(hx, hy, og.hz) * slack)
+    # diagnostic (not asserted): the same comparison with the oracle rounding the GPU's exported fp32 coefficients isolates the fp32 arithmetic
+    coef32 = api.gridff_grid_export(g).cpu().numpy()
+    hg_same = orc.OracleGrid(coef32.astype(np.float16).astype(np.float64), og.Lx, og.Ly, og.z0, og.hz)
+    Es, Fs = orc.interp(hg_same, pos, cf)
     # and the price of fp16 against the full-precision spline (reported)
     Ef, Ff = orc.interp(og, pos, cf)
-    print("fp16 store vs fp64 spline: median rel E err %.2e, max %.2e; max |dF| %.2e eV/A"
-          % (np.median(np.abs(E - Ef) / den), (np.abs(E - Ef) / den).max(), np.abs(F - Ff).max()))
+    print("fp16 store: %.1f %% of the points at the plain tolerance; vs the oracle rounding the exported coefficients: max rel E %.2e, max |dF| %.2e; "
+          "vs the fp64 spline: median rel E err %.2e, max %.2e; max |dF| %.2e eV/A"
+          % (100 * (slack == 0).mean(), (np.abs(E - Es) / den).max(), np.abs(F - Fs).max(),
+             np.median(np.abs(E - Ef) / den), (np.abs(E - Ef) / den).max(), np.abs(F - Ff).max()))
     with pytest.raises(api.GridffError):
         api.gridff_grid_export(gh)
 
