@@ -381,7 +381,7 @@ def run_gridff(args, emit=True):
     # L2 read bandwidth measured live with the library's probe over a buffer the size of the coefficient store (stays in L2)
     probe = torch.empty(min(max(sb, 16 << 20), 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)
     l2 = {}
-    for mode, key in ((0, "stream"), (1, "rows64")):
+    for mode, key in ((0, "stream"), (1, "rows64"), (2, "lines128")):
         api.gridff_probe_read(probe, iters=100, mode=mode); torch.cuda.synchronize()        # warm: clocks up, buffer in L2
         best = 0.0
         for _ in range(10):
@@ -576,7 +576,7 @@ def run_eval(args, emit=True):
     def l2_probe(nbytes):
         probe = torch.empty(min(max(nbytes, 16 << 20), 96 << 20), dtype=torch.uint8, device="cuda"); probe.fill_(1)     # >= 16 MB: a smaller buffer cannot occupy every SM
         out = {}
-        for mode, key in ((0, "stream"), (1, "rows64")):
+        for mode, key in ((0, "stream"), (1, "rows64"), (2, "lines128")):
             api.gridff_probe_read(probe, iters=100, mode=mode); torch.cuda.synchronize()    # warm: clocks up, buffer in L2
             best = 0.0
             for _ in range(10):

@@ -279,8 +279,9 @@ int gridff_run_replicas_host(const gridff_grid* grid, const gridff_molecule* mol
  * Measurement helpers (roofline denominators; not part of the method)
  * --------------------------------------------------------------------------------------------------------- */
 
-/* Read `bytes` of d_buf `iters` times with coalesced 16-byte loads (mode 0) or with the 64-byte-row gather pattern of
- * the stencil at random offsets (mode 1); one launch.  d_sink: >= 4 bytes.  Used to measure L2 / HBM read bandwidth. */
+/* Read `bytes` of d_buf `iters` times with coalesced 16-byte loads (mode 0), with the 64-byte-row gather pattern of
+ * the z-fastest stencil at random 16-byte offsets (mode 1), or as whole aligned 128-byte lines at random positions, the
+ * micro-brick stencil's granule (mode 2); one launch.  d_sink: >= 4 bytes.  Used to measure L2 / HBM read bandwidth. */
 int gridff_probe_read(const void* d_buf, size_t bytes, int iters, int mode, void* d_sink, void* cuda_stream);
 
 /* Number of kernel launches the library has enqueued since it was loaded (for bench.py's gpu_launches). */

@@ -144,13 +144,15 @@ __global__ void __launch_bounds__(256) k_probe_stream(const float4* __restrict__
     if (acc == 1.2345678e-30f) *sink = acc;
 }
 
-// 4 lanes read one 64-byte row at a random 16-byte-aligned offset (the stencil's access granule)
+// LANES = 4: 4 lanes read one 64-byte row at a random 16-byte-aligned offset (the z-fastest stencil's access granule);
+// LANES = 8: 8 lanes read one whole, aligned 128-byte line at a random position (the micro-brick stencil's granule)
+template <int LANES>
 __global__ void __launch_bounds__(256) k_probe_rows(const float4* __restrict__ buf, size_t n16, int iters, float* sink) {
     float acc = 0.f;
-    const unsigned quad = (blockIdx.x * blockDim.x + threadIdx.x) >> 2, k = threadIdx.x & 3;
-    const unsigned nquads = (gridDim.x * blockDim.x) >> 2;
-    const size_t rows = n16 / 4;                   // rows of 64 B to read per pass
-    const unsigned span = (unsigned)(n16 - 4);
+    const unsigned quad = (blockIdx.x * blockDim.x + threadIdx.x) / LANES, k = threadIdx.x % LANES;
+    const unsigned nquads = (gridDim.x * blockDim.x) / LANES;
+    const size_t rows = n16 / LANES;               // rows to read per pass
+    const unsigned span = (unsigned)(n16 - LANES);
     for (int it = 0; it < iters; ++it) {
         for (size_t r = quad; r < rows; r += (size_t)nquads * 4) {
             unsigned h = hash32((unsigned)r * 2654435761u + (unsigned)it);
@@ -158,7 +160,7 @@ __global__ void __launch_bounds__(256) k_probe_rows(const float4* __restrict__ b
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
                 const size_t rr = r + (size_t)u * nquads;
-                if (rr < rows) { v[u] = __ldcg(buf + (size_t)(h % span) + k); } else v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+                if (rr < rows) { const size_t o = (size_t)(h % span); v[u] = __ldcg(buf + (LANES == 8 ? (o & ~(size_t)7) : o) + k); } else v[u] = make_float4(0.f, 0.f, 0.f, 0.f);
                 h = hash32(h + 0x9e3779b9u);
             }
             acc += (v[0].x + v[1].y) + (v[2].z + v[3].w);
@@ -299,13 +301,14 @@ int gridff_eval_host(const gridff_grid* grid, long long n, const float* h_pos, c
 int gridff_probe_read(const void* d_buf, size_t bytes, int iters, int mode, void* d_sink, void* cuda_stream) {
     if (!d_buf || !d_sink || bytes < 4096 || iters < 1) { set_error("bad probe arguments"); return GRIDFF_EINVAL; }
     if ((uintptr_t)d_buf & 15) { set_error("d_buf must be 16-byte aligned"); return GRIDFF_EINVAL; }
-    if (bytes / 16 > 0xFFFFFFF0ull && mode == 1) { set_error("row probe supports < 64 GB"); return GRIDFF_EINVAL; }
+    if (bytes / 16 > 0xFFFFFFF0ull && mode >= 1) { set_error("row probe supports < 64 GB"); return GRIDFF_EINVAL; }
     int dev = 0, sms = 148;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (mode == 0) k_probe_stream<<<sms * 8, 256, 0, st>>>((const float4*)d_buf, bytes / 16, iters, (float*)d_sink);
-    else if (mode == 1) k_probe_rows<<<sms * 8, 256, 0, st>>>((const float4*)d_buf, bytes / 16, iters, (float*)d_sink);
+    else if (mode == 1) k_probe_rows<4><<<sms * 8, 256, 0, st>>>((const float4*)d_buf, bytes / 16, iters, (float*)d_sink);
+    else if (mode == 2) k_probe_rows<8><<<sms * 8, 256, 0, st>>>((const float4*)d_buf, bytes / 16, iters, (float*)d_sink);
     else { set_error("unknown probe mode %d", mode); return GRIDFF_EINVAL; }
     GRIDFF_LAUNCH_CHECK("gridff_probe_read");
     return GRIDFF_OK;
