@@ -196,8 +196,9 @@ typedef struct {
                                  3 = 2 + the folded stencils cached in shared memory and re-gathered only when an atom changes cell.
                                  Molecules of 33-64 atoms: variants 1, 2 put two atoms on a lane; variant 3 puts the replica on a pair of warps
                                  (one atom per lane); variant 4 = variant 3's stencil cache on ONE warp with two atoms per lane (the older kernel, kept
-                                 for the design comparison; for <= 32 atoms it is variant 3).  All variants compute the same forces; they differ in
-                                 rounding order only. */
+                                 for the design comparison; for <= 32 atoms it is variant 3); variant 5 = variant 3 with the pair loop of molecules of
+                                 <= 32 atoms as a full shell with a warp-uniform partner instead of the half shell on a ring (design comparison: slower;
+                                 for 33-64 atoms it is variant 3).  All variants compute the same forces; they differ in rounding order only. */
     /* SURVEY.md §8(f) rows 1-2 (0 / unset = off) */
     float temperature;        /* K, kind 2 */
     float gamma;              /* friction 1/fs, kind 2: per step  B: v += dt/2 a;  A: x += dt/2 v;  O: v = c1 v + c2 sqrt(kT/m) xi;  A;  F(x);  B,

@@ -5,13 +5,16 @@
 // accelerator moves: one `cp.async.bulk.tensor.3d` (SASS UTMALDG) per point lands the box in shared memory and signals an mbarrier, without
 // occupying the LSU / L1 data pipe that bounds the warp-cooperative LDG gather (k_eval_coop: one L1 cycle per distinct 128-byte line, 22 per
 // stencil).  The tensor is described to the TMA unit as fp32 elements {nzp * 4, ny + 3, nx + 3} (z and channel merged: TMA has no
-// 16-byte element type), box {16, 4, 4}, no swizzle, no L2 promotion (a 64-byte row needs 2-3 sectors, not whole 128-byte lines).
+// 16-byte element type), box {16, 4, 4}, no swizzle, 64-byte L2 promotion.  The 8-copy micro-brick store (gridff_derive.cu) is a 5-D tensor
+// {32 floats = a brick, nbz, nby, nbx, 8 copies}; a stencil is the box {32, 2, 2, 2, 1} in the copy of its corner's parity: 8 whole 128-byte lines
+// (UTMALDG.5D) — the template parameter BRICKS.
 //
-// A warp owns 32 consecutive points and walks over its tiles persistently.  Per tile: the two halves (16 points, 16 KB each) arrive in two raw
-// buffers with their own mbarriers; the warp folds each half with the points' channel factors into the same XOR-swizzled 8 KB tile that
-// k_eval_coop builds (lanes read consecutive 16-byte chunks of the raw box: conflict-free), re-arms the half's buffer with the NEXT tile's
-// boxes, and finally every lane contracts its own point (interp_tile).  The folded tile and the contraction are bit-identical to k_eval_coop's,
-// so variant 3 returns exactly variant 2's numbers (test).  Up to 32 KB per warp and 160 KB per SM are in flight behind the arithmetic.
+// A warp owns 32 consecutive points and walks over its tiles persistently.  Per tile the boxes arrive in 4 groups of 8 points that alternate
+// between two raw buffers of 8 KB with their own mbarriers; the warp folds each group with the points' channel factors into the same XOR-swizzled
+// 8 KB tile that k_eval_coop builds (lanes read consecutive 16-byte chunks of the raw box: conflict-free), re-arms the buffer with the group
+// after next (of this tile or of the warp's next one), and finally every lane contracts its own point (interp_tile).  The folded tile and the
+// contraction are bit-identical to k_eval_coop's, so variant 3 returns exactly variant 2's numbers (test).  24.6 KB per warp: 8 warps and 128 KB
+// in flight per SM behind the arithmetic (16-point groups, 41 KB and 5 warps: 10 % slower on the HBM-bound brick store, profiles/r2_hbm.md).
 #include "gridff_interp.cuh"
 #include <cuda.h>
 #include <stdio.h>
