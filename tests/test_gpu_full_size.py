@@ -100,6 +100,14 @@ def test_config4_full_size_sampled_points_and_order(api, orc):
     perm = inputs.morton_order(d_pos, d["Lx"], d["Ly"], d["z_ref"] + d["z_lo"], 113, 113, d["spacing"], xp=torch)
     Es, Fs = api.gridff_eval(g, d_pos[perm].contiguous(), d_coef[perm].contiguous())
     assert bool(torch.equal(Es, E[perm])) and bool(torch.equal(Fs, F[perm]))
+    # the 8-copy micro-brick store of the same grid (180 MB: beyond the L2, so the default takes the device-side choice: 5-D TMA boxes for the
+    # random order, the LDG gather for the sorted one) returns the same numbers bit for bit, in the launch shape bench.py times
+    gb = api.gridff_grid_derive(g, api.LAYOUT_MBRICK8)
+    Eb, Fb = api.gridff_eval(gb, d_pos, d_coef)
+    assert bool(torch.equal(Eb, E)) and bool(torch.equal(Fb, F))
+    Eb, Fb = api.gridff_eval(gb, d_pos[perm].contiguous(), d_coef[perm].contiguous())
+    assert bool(torch.equal(Eb, Es)) and bool(torch.equal(Fb, Fs))
+    gb.free(); del gb, Eb, Fb
     # the spatial sort did what it says: consecutive points share a cell far more often than in random order
     cell = lambda p: (torch.floor(p[:, 0] / d["Lx"] * 113) * 113 + torch.floor(p[:, 1] / d["Ly"] * 113)).long()
     c_s = cell(d_pos[perm][: 1 << 20]); c_r = cell(d_pos[: 1 << 20])
