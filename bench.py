@@ -65,7 +65,7 @@ def workload(args):
     nx, ny, nz = inputs.grid_dims(cfg["desc"])
     name = {0: "config0: NaCl(001) 4x4 slab, 2 channels, 64 x benzene, FIRE x 1000",
             2: "config2: config1 grid, 16384 x 60-atom flexible chain, FIRE (dt0 0.5 fs, dt_max 20 fs, displacement cap 0.1 A per step) to 1e-3 eV/A, "
-               "cap 20000 iterations per launch, + Philox restart; batches above 256 replicas start from 256 seeded conformers",
+               "cap 20000 iterations per launch, + Philox restart; every replica starts from its own seeded clash-free random dihedrals",
             1: "config1: NaCl(001) 4x4 slab + Coulomb, 4096 x 30-atom aromatic, VV dt 0.5 fs x 10000",
             3: "config3: 40x40 Å slab, 400x400x150x4 grid (384 MB), 8192 x 30-atom aromatic, VV x 5000"}[args.config]
     return cfg, md, (nx, ny, nz), name

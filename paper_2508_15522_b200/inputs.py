@@ -320,43 +320,78 @@ def _random_rotations(rng, n):
                      np.stack([2 * (x * z - y * w), 2 * (y * z + x * w), 1 - 2 * (x * x + y * y)], -1)], 1)
 
 
-def _twist(pos, topo, rng, clash=0.6, tries=256):
-    """random dihedral about every rotatable bond; re-draw while a non-excluded pair is closer than
-    clash * (R_i + R_j); if no draw passes, the least-clashing one is kept."""
+def _twist_grow(ref, topo, rng, n_rep, clash=0.6, tries=64, restarts=64):
+    """n_rep conformers of the template, one random dihedral about every rotatable bond, free of clashes (no non-excluded pair closer than
+    clash * (R_i + R_j)), by chain growth, vectorised over the replicas: the bonds are taken from the fixed core outwards (largest turning
+    side first); each dihedral is drawn ~ U(-pi, pi) and re-drawn (up to `tries` times) while the atoms it puts in their final place clash
+    with atoms already in theirs; a replica that finds no angle starts again from the template (up to `restarts` times).  The turning sides
+    of the bonds must be nested or disjoint (a tree).  -> float64 [n_rep][n][3]"""
     n = topo["n_atoms"]
-    Rsum = topo["lj_R"][:, None].astype(np.float64) + topo["lj_R"][None, :]
-    free = topo["excl"] == 0
-    best, best_gap = None, -1.0
-    for _ in range(tries):
-        p = pos.copy()
-        for b, (j0, j1) in enumerate(topo["rot_bond"]):
-            ang = rng.uniform(-math.pi, math.pi)
-            ax = p[j1] - p[j0]; ax /= np.linalg.norm(ax)
-            sel = topo["rot_mask"][b].astype(bool)
-            v = p[sel] - p[j0]
-            p[sel] = p[j0] + v * math.cos(ang) + np.cross(ax, v) * math.sin(ang) + np.outer(v @ ax, ax) * (1 - math.cos(ang))
-        d = np.linalg.norm(p[:, None, :] - p[None, :, :], axis=-1)
-        gap = float(np.min(np.where(free, d / Rsum, np.inf)))
-        if gap >= clash:
-            return p
-        if gap > best_gap:
-            best, best_gap = p, gap
-    return best
+    lim2 = ((topo["lj_R"][:, None].astype(np.float64) + topo["lj_R"][None, :]) * clash) ** 2
+    free = (topo["excl"] == 0) & (topo["excl"].T == 0) & ~np.eye(n, dtype=bool)
+    masks = [np.asarray(m, bool) for m in topo["rot_mask"]]
+    order = sorted(range(len(masks)), key=lambda b: -int(masks[b].sum()))
+    # an atom's position depends on dihedral b iff it is on b's turning side and not on its axis (the far bond atom j1 turns with itself but
+    # stays put); it is in its final place after the last bond, in this order, that moves it
+    last = np.full(n, -1)
+    for k, b in enumerate(order):
+        moved = masks[b].copy(); moved[int(topo["rot_bond"][b][1])] = False
+        last[moved] = k
+    steps, done = [], last < 0
+    for k, b in enumerate(order):
+        new = last == k
+        old_idx, new_idx = np.nonzero(done)[0], np.nonzero(new)[0]
+        pi, pj = np.meshgrid(new_idx, old_idx, indexing="ij")
+        keep = free[pi, pj]
+        # pairs among the new atoms themselves are rigid with respect to this rotation: nothing to test
+        steps.append((b, np.nonzero(masks[b])[0], pi[keep], pj[keep], lim2[pi, pj][keep]))
+        done = done | new
+    ref = np.asarray(ref, np.float64)
+    out = np.broadcast_to(ref, (n_rep, n, 3)).copy()
+    todo = np.arange(n_rep)
+    for _ in range(restarts):
+        p = np.broadcast_to(ref, (len(todo), n, 3)).copy()
+        alive = np.ones(len(todo), bool)
+        for b, sel, pi, pj, l2 in steps:
+            j0, j1 = (int(v) for v in topo["rot_bond"][b])
+            need = alive.copy()
+            base = p[:, sel, :].copy()
+            for _t in range(tries):
+                idx = np.nonzero(need)[0]
+                if len(idx) == 0:
+                    break
+                ang = rng.uniform(-math.pi, math.pi, len(idx))
+                o = p[idx, j0, :][:, None, :]
+                ax = p[idx, j1, :] - p[idx, j0, :]; ax /= np.linalg.norm(ax, axis=1, keepdims=True)
+                axb = ax[:, None, :]
+                v = base[idx] - o
+                c, s_ = np.cos(ang)[:, None, None], np.sin(ang)[:, None, None]
+                q = p[idx].copy()
+                q[:, sel, :] = o + v * c + np.cross(axb, v) * s_ + axb * np.sum(v * axb, axis=2, keepdims=True) * (1 - c)
+                d = q[:, pi, :] - q[:, pj, :]
+                ok = np.all(np.einsum("kij,kij->ki", d, d) >= l2[None, :], axis=1) if len(pi) else np.ones(len(idx), bool)
+                p[idx[ok]] = q[ok]
+                need[idx[ok]] = False
+            alive &= ~need
+        out[todo[alive]] = p[alive]
+        todo = todo[~alive]
+        if len(todo) == 0:
+            return out
+    raise RuntimeError("chain growth found no clash-free conformer for %d replicas" % len(todo))
 
 
-def place_replicas(topo, n_rep, Lx, Ly, z_ref, seed, z_lo=3.0, z_hi=6.0, z_min=2.0, twist=False, twist_pool=256):
+def place_replicas(topo, n_rep, Lx, Ly, z_ref, seed, z_lo=3.0, z_hi=6.0, z_min=2.0, twist=False):
     """centroid x,y ~ U(0,L), orientation uniform on SO(3), centroid z ~ U(z_lo, z_hi) above z_ref, lifted so the
-    lowest atom is >= z_min above z_ref.  Returns float32 [n_rep][n][3].  With `twist`, every replica gets its own clash-free random
-    dihedrals while n_rep <= twist_pool; larger batches draw twist_pool conformers and replica r takes conformer r mod twist_pool
-    (its orientation and placement stay its own) — the clash-free re-draws are a Python loop, ~80 ms each."""
+    lowest atom is >= z_min above z_ref.  Returns float32 [n_rep][n][3].  With `twist`, EVERY replica gets its own clash-free random
+    dihedrals about the rotatable bonds (config 2: "random initial dihedrals"; _twist_grow)."""
     rng = np.random.default_rng(seed)
     n = topo["n_atoms"]
     ref = np.asarray(topo["ref_pos"], dtype=np.float64)
     rots = _random_rotations(rng, n_rep)
+    conf = _twist_grow(ref, topo, rng, n_rep) if twist else None
     out = np.zeros((n_rep, n, 3))
-    pool = [_twist(ref, topo, rng) for _ in range(twist_pool)] if (twist and n_rep > twist_pool) else None
     for r in range(n_rep):
-        p = pool[r % twist_pool] if pool is not None else (_twist(ref, topo, rng) if twist else ref)
+        p = conf[r] if twist else ref
         p = (p - p.mean(axis=0)) @ rots[r].T
         p = p + np.array([rng.uniform(0, Lx), rng.uniform(0, Ly), z_ref + rng.uniform(z_lo, z_hi)])
         lift = z_ref + z_min - p[:, 2].min()
