@@ -55,6 +55,8 @@ def parse():
     ap.add_argument("--c4-store", default="fp32", choices=["fp32", "half", "trilinear", "bricks", "bricks2", "bricks8"],
                     help="config 4: coefficient store read by gridff_eval: the fp32 spline z-fastest (default), fp16 coefficients, the paper's trilinear foil "
                          "(SURVEY §8(f)3), or the fp32 spline in 2x2x2-node bricks of 128 B, 1 / 2 / 8 shifted copies (the layouts for stores beyond the L2)")
+    ap.add_argument("--binned", action="store_true", help="config 4: time gridff_eval_binned (device-side counting sort of the points by cell block, then the "
+                                                          "gather) instead of gridff_eval; z-fastest fp32 store only")
     ap.add_argument("--sweep", action="store_true", help="config 4: also time the grid-size x order sweep (32^3 ... 512x512x256)")
     return ap.parse_args()
 
@@ -452,9 +454,10 @@ def also_entries(args):
             ("config4_sorted", dict(config=4, order="sorted", c4_grid="config1", log2_points=26)),
             ("config4_hbm_512x512x256_random", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25)),
             ("config4_hbm_512x512x256_sorted", dict(config=4, order="sorted", c4_grid="512x512x256", log2_points=25)),
-            ("config4_hbm_512x512x256_random_bricks8", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25, c4_store="bricks8"))]
+            ("config4_hbm_512x512x256_random_bricks8", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25, c4_store="bricks8")),
+            ("config4_hbm_512x512x256_random_binned", dict(config=4, order="random", c4_grid="512x512x256", log2_points=25, binned=True))]
     for key, kw in todo:
-        a = argparse.Namespace(**dict(dict(base, c4_store="fp32", sweep=False), **kw))
+        a = argparse.Namespace(**dict(dict(base, c4_store="fp32", sweep=False, binned=False), **kw))
         t0 = time.perf_counter()
         try:
             r = run_eval(a, emit=False) if a.config == 4 else run_gridff(a, emit=False)
@@ -586,12 +589,22 @@ def run_eval(args, emit=True):
             out[key] = best
         return out
 
+    binned_work = {}
+
     def time_eval(g, d_pos, d_coef, d_E, d_F, reps, warm):
         ts = []
+        binned = getattr(args, "binned", False) and args.c4_store == "fp32"
+        if binned and "w" not in binned_work:
+            binned_work["w"] = torch.empty(int(api._lib.gridff_eval_binned_work_bytes(g.handle, d_pos.shape[0])), dtype=torch.uint8, device="cuda")
         for it in range(warm + reps):
             flush.fill_(1)
             a, b = ev(), ev()
-            a.record(stream); api.gridff_eval(g, d_pos, d_coef, d_E=d_E, d_F=d_F, variant=args.variant or None); b.record(stream); b.synchronize()
+            a.record(stream)
+            if binned:
+                api.gridff_eval_binned(g, d_pos, d_coef, d_E=d_E, d_F=d_F, d_work=binned_work["w"])
+            else:
+                api.gridff_eval(g, d_pos, d_coef, d_E=d_E, d_F=d_F, variant=args.variant or None)
+            b.record(stream); b.synchronize()
             if it >= warm:
                 ts.append(a.elapsed_time(b))
         return ts
@@ -663,6 +676,8 @@ def run_eval(args, emit=True):
         tkey += "_sorted"
     if args.c4_store != "fp32":
         tkey += "_" + args.c4_store
+    if getattr(args, "binned", False):
+        tkey += "_binned"
     fits, ach, peak = roof(sb, n, kern_ms, l2)
     traffic = None
     try:
@@ -725,7 +740,7 @@ def run_eval(args, emit=True):
         "metric": C4_METRIC, "value": value, "unit": C4_UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": "config4: 2^%d uniformly random points, %s, 3-channel E + analytic gradient" % (args.log2_points, name),
-                   "grid": list(dims), "store": args.c4_store, "store_bytes": sb, "points_per_gpu": n, "order": args.order, "parallelism": "points only (no collective)",
+                   "grid": list(dims), "store": args.c4_store, "binned": bool(getattr(args, "binned", False)), "store_bytes": sb, "points_per_gpu": n, "order": args.order, "parallelism": "points only (no collective)",
                    "l2_flush_between_steps": True, "step": "gridff_eval over all points (grid built before the timed region)"},
         "clocks": clocks, "e2e": {"value": e2e_value, "unit": C4_UNIT, "h2d_bytes_per_step": n * 28, "d2h_bytes_per_step": n * 16},
         "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "sweep": sweep})

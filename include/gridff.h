@@ -147,6 +147,15 @@ int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const 
 int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
                         float* d_E, float* d_F, int variant, void* cuda_stream);
 
+/* Same results as gridff_eval (bit for bit) for SCATTERED points on a z-fastest store that does not fit the L2 ("limited by global
+ * memory access"): the points are first counting-sorted on the device by blocks of 4 x 4 x 8 cells (one atomic pass for count and rank, a scan,
+ * a scatter of 32-byte point records), evaluated block by block, and the results gathered back to the points' own indices — neighbouring points
+ * then share stencil lines in L1 / L2 as spatially sorted input does, without any extra copy of the grid.  d_work needs gridff_eval_binned_work_bytes(grid, n)
+ * bytes (52 n + 4 per bin), 256-byte aligned; n < 2^32 - 16.  The order inside a bin depends on the atomics' order; the results do not. */
+size_t gridff_eval_binned_work_bytes(const gridff_grid* grid, long long n);
+int gridff_eval_binned(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
+                       float* d_E, float* d_F, void* d_work, size_t work_bytes, void* cuda_stream);
+
 /* Same through HOST buffers: copies pos/coef to d_work, evaluates, copies E/F back, synchronises the stream.
  * d_work needs gridff_eval_work_bytes(n) bytes.  The work is pipelined in chunks of 2^22 points over two library-owned copy streams
  * and the caller's stream (upload of chunk c+1, kernel of chunk c and download of chunk c-1 overlap); the overlap needs pinned

@@ -82,6 +82,8 @@ _SIG = {
     "gridff_atom_coefs": (_i, [C.c_double, _i, _vp, _vp, _vp, _vp]),
     "gridff_eval": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp]),
     "gridff_eval_variant": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _i, _vp]),
+    "gridff_eval_binned_work_bytes": (_sz, [_vp, _ll]),
+    "gridff_eval_binned": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "gridff_eval_work_bytes": (_sz, [_ll]),
     "gridff_eval_host": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "gridff_molecule_bytes": (_sz, [_P(Topology)]),
@@ -268,6 +270,20 @@ def gridff_eval(grid, d_pos, d_coef, d_E=None, d_F=None, stream=None, variant=No
         _check(_lib.gridff_eval(grid.handle, n, _dptr(d_pos), _dptr(d_coef), _dptr(d_E), _dptr(d_F), _stream(stream)))
     else:
         _check(_lib.gridff_eval_variant(grid.handle, n, _dptr(d_pos), _dptr(d_coef), _dptr(d_E), _dptr(d_F), int(variant), _stream(stream)))
+    return d_E, d_F
+
+
+def gridff_eval_binned(grid, d_pos, d_coef, d_E=None, d_F=None, d_work=None, stream=None):
+    """gridff_eval for scattered points on a store beyond the L2: the points are counting-sorted by cell block on the device first.
+    Returns (E [n], F [n][3]) — the same numbers as gridff_eval."""
+    n = d_pos.shape[0]
+    if d_E is None:
+        d_E = torch.empty(n, dtype=torch.float32, device="cuda")
+    if d_F is None:
+        d_F = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+    if d_work is None:
+        d_work = _alloc(int(_lib.gridff_eval_binned_work_bytes(grid.handle, n)))
+    _check(_lib.gridff_eval_binned(grid.handle, n, _dptr(d_pos), _dptr(d_coef), _dptr(d_E), _dptr(d_F), _dptr(d_work), d_work.numel(), _stream(stream)))
     return d_E, d_F
 
 

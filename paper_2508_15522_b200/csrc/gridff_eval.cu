@@ -25,8 +25,11 @@ __global__ void __launch_bounds__(128) k_eval_direct(GridGeom g, long long n, co
 constexpr int kEvalWarps = 4;
 
 // `choice` (may be NULL): device word written by k_eval_classify; the kernel runs only when it holds kChoiceCoop
+// `rec` (may be NULL; gridff_eval_binned): the points as 32-byte records {x, y, z, index}, {coef} in bin order; the results then go, as
+// float4 {E, Fx, Fy, Fz} per slot, to `out4` (k_bin_gather_out hands them to the points' own indices)
 __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef,
-                                                               float* __restrict__ E, float* __restrict__ F, const unsigned* __restrict__ choice) {
+                                                               float* __restrict__ E, float* __restrict__ F, const unsigned* __restrict__ choice,
+                                                               const float4* __restrict__ rec, float4* __restrict__ out4) {
     if (choice && *choice != kChoiceCoop) return;
     __shared__ __align__(16) float s_tile[kEvalWarps][32 * 64];
     __shared__ __align__(16) float4 s_cf[kEvalWarps][32];
@@ -36,7 +39,10 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
     Stencil s; s.base = kNoStencil; s.tx = s.ty = s.tz = 0.f;
     float4 cf = make_float4(0.f, 0.f, 0.f, 0.f);
     int ix = 0, iy = 0, iz = 0;
-    if (p < n) { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz); cf = coef[p]; }
+    if (p < n) {
+        if (rec) { const float4 a = rec[2 * p]; s = locate(g, a.x, a.y, a.z, ix, iy, iz); cf = rec[2 * p + 1]; }
+        else { s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz); cf = coef[p]; }
+    }
     s_base[w][lane] = s.base; s_cf[w][lane] = cf;
     warp_sync();
     float* tile = s_tile[w];
@@ -59,8 +65,73 @@ __global__ void __launch_bounds__(kEvalWarps * 32) k_eval_coop(GridGeom g, long 
     if (p >= n) return;
     float e, fx, fy, fz;
     interp_tile(g, s, lane, tile, e, fx, fy, fz);
+    if (out4) { out4[p] = make_float4(e, fx, fy, fz); return; }
     if (E) E[p] = e;
     if (F) { F[3 * p] = fx; F[3 * p + 1] = fy; F[3 * p + 2] = fz; }
+}
+
+// ---- gridff_eval_binned: a counting sort of the points by coarse cell block, so that scattered points are gathered with the locality of sorted ones ----
+// Bins are blocks of 4 x 4 x 8 cells in [x][y][z] order (z fastest, like the store); points above the domain go to one extra bin at the end.
+constexpr int kBinX = 2, kBinY = 2, kBinZ = 3;            // log2 of the block's cells per axis
+__device__ __forceinline__ unsigned bin_of(const GridGeom& g, const float* __restrict__ pos, long long p, int nby, int nbz, unsigned n_bins) {
+    int ix, iy, iz;
+    const Stencil s = locate(g, pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], ix, iy, iz);
+    if (s.base == kNoStencil) return n_bins - 1;
+    return (unsigned)(((ix >> kBinX) * nby + (iy >> kBinY)) * nbz + (iz >> kBinZ));
+}
+// pass 1: count[bin]++, the value before the increment is the point's rank within its bin
+__global__ void __launch_bounds__(256) k_bin_count(GridGeom g, long long n, const float* __restrict__ pos, int nby, int nbz, unsigned n_bins,
+                                                   unsigned* __restrict__ count, unsigned* __restrict__ rank) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    rank[p] = atomicAdd(count + bin_of(g, pos, p, nby, nbz, n_bins), 1u);
+}
+// pass 2: exclusive scan of the counts in place: one block walks over tiles of 1024 counts (coalesced), scanning each with warp shuffles
+__global__ void __launch_bounds__(1024) k_bin_scan(unsigned n_bins, unsigned* __restrict__ count) {
+    __shared__ unsigned s_warp[32];
+    __shared__ unsigned s_run;
+    const unsigned lane = threadIdx.x & 31u, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_run = 0u;
+    __syncthreads();
+    unsigned next = threadIdx.x < n_bins ? count[threadIdx.x] : 0u;
+    for (unsigned t0 = 0; t0 < n_bins; t0 += 1024u) {
+        const unsigned b = t0 + threadIdx.x;
+        const unsigned c = next;
+        next = b + 1024u < n_bins ? count[b + 1024u] : 0u;     // the next tile's counts are on their way while this one is scanned
+        unsigned inc = c;
+#pragma unroll
+        for (unsigned o = 1; o < 32u; o <<= 1) { const unsigned v = __shfl_up_sync(0xFFFFFFFFu, inc, o); if (lane >= o) inc += v; }
+        if (lane == 31u) s_warp[w] = inc;
+        __syncthreads();
+        unsigned wsum = s_warp[lane];                          // every warp scans the 32 warp totals
+#pragma unroll
+        for (unsigned o = 1; o < 32u; o <<= 1) { const unsigned v = __shfl_up_sync(0xFFFFFFFFu, wsum, o); if (lane >= o) wsum += v; }
+        const unsigned before = __shfl_sync(0xFFFFFFFFu, wsum, w) - s_warp[w], total = __shfl_sync(0xFFFFFFFFu, wsum, 31);
+        const unsigned run = s_run;
+        if (b < n_bins) count[b] = run + before + inc - c;
+        __syncthreads();                                       // s_warp and s_run have been read
+        if (threadIdx.x == 0) s_run = run + total;
+        __syncthreads();
+    }
+}
+// pass 3: slot = offset[bin] + rank; the point's 32-byte record {x, y, z, index}, {coef} goes to rec[slot] (one whole sector), slot to rank[p]
+__global__ void __launch_bounds__(256) k_bin_scatter(GridGeom g, long long n, const float* __restrict__ pos, const float4* __restrict__ coef, int nby, int nbz,
+                                                     unsigned n_bins, const unsigned* __restrict__ offset, unsigned* __restrict__ rank, float4* __restrict__ rec) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const unsigned slot = offset[bin_of(g, pos, p, nby, nbz, n_bins)] + rank[p];
+    rank[p] = slot;
+    rec[2 * (size_t)slot] = make_float4(pos[3 * p], pos[3 * p + 1], pos[3 * p + 2], __uint_as_float((unsigned)p));
+    rec[2 * (size_t)slot + 1] = coef[p];
+}
+// pass 5: the results back to the points' own indices (random 16-byte reads, coalesced writes)
+__global__ void __launch_bounds__(256) k_bin_gather_out(long long n, const unsigned* __restrict__ slot, const float4* __restrict__ out4,
+                                                        float* __restrict__ E, float* __restrict__ F) {
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const float4 o = __ldcg(out4 + slot[p]);
+    if (E) E[p] = o.x;
+    if (F) { F[3 * p] = o.y; F[3 * p + 1] = o.z; F[3 * p + 2] = o.w; }
 }
 
 // Which kernel for a store that does not fit the L2?  Scattered points: the TMA box kernel (DRAM-bound, it keeps more bytes in flight: +26 %);
@@ -230,7 +301,7 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
         }
         const long long per_block = kEvalWarps * 32;
         e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef, d_E, d_F,
-                               choice);
+                               choice, (const float4*)nullptr, (float4*)nullptr);
     } else { set_error("unknown eval variant %d", variant); return GRIDFF_EINVAL; }
     count_launch();
     if (e != cudaSuccess) return cuda_fail(e, "gridff_eval launch");
@@ -239,6 +310,57 @@ int gridff_eval_variant(const gridff_grid* grid, long long n, const float* d_pos
 
 int gridff_eval(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, void* cuda_stream) {
     return gridff_eval_variant(grid, n, d_pos, d_coef, d_E, d_F, 0, cuda_stream);
+}
+
+static unsigned binned_bins(const GridGeom& G, int& nby, int& nbz) {
+    const int nbx = (G.nx + (1 << kBinX) - 1) >> kBinX;
+    nby = (G.ny + (1 << kBinY) - 1) >> kBinY; nbz = (G.nz + (1 << kBinZ) - 1) >> kBinZ;
+    return (unsigned)(nbx * nby * nbz) + 1u;                    // + the bin of the points above the domain
+}
+
+size_t gridff_eval_binned_work_bytes(const gridff_grid* grid, long long n) {
+    if (!grid || n < 0) return 0;
+    int nby, nbz;
+    const size_t bins = binned_bins(grid->geom, nby, nbz);
+    return (((size_t)n * 4 + 255) & ~(size_t)255) + (size_t)n * 32 + (((size_t)n * 16 + 255) & ~(size_t)255) + ((bins * 4 + 255) & ~(size_t)255) + 256;
+}
+
+int gridff_eval_binned(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F,
+                       void* d_work, size_t work_bytes, void* cuda_stream) {
+    if (!grid) { set_error("grid is NULL"); return GRIDFF_EINVAL; }
+    if (n < 0) { set_error("n < 0"); return GRIDFF_EINVAL; }
+    if (n == 0) return GRIDFF_OK;
+    if (n > 0xFFFFFFF0ll) { set_error("gridff_eval_binned takes at most 2^32 - 16 points per call"); return GRIDFF_EUNSUPPORTED; }
+    if (!d_pos || !d_coef) { set_error("d_pos / d_coef is NULL"); return GRIDFF_EINVAL; }
+    if ((uintptr_t)d_coef & 15) { set_error("d_coef must be 16-byte aligned"); return GRIDFF_EINVAL; }
+    if (grid->geom.layout != GRIDFF_LAYOUT_ZFAST) { set_error("gridff_eval_binned reads the z-fastest store"); return GRIDFF_EUNSUPPORTED; }
+    if (!d_work || work_bytes < gridff_eval_binned_work_bytes(grid, n)) { set_error("d_work too small"); return GRIDFF_ESIZE; }
+    if ((uintptr_t)d_work & 255) { set_error("d_work must be 256-byte aligned"); return GRIDFF_EINVAL; }
+    const GridGeom& G = grid->geom;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int nby, nbz;
+    const unsigned n_bins = binned_bins(G, nby, nbz);
+    const size_t np4 = ((size_t)n * 4 + 255) & ~(size_t)255;
+    unsigned* rank = (unsigned*)d_work;                                   // rank within the bin, then the slot
+    float4* rec = (float4*)((char*)d_work + np4);                          // [n] x 32 B
+    float4* out4 = (float4*)((char*)d_work + np4 + (size_t)n * 32);        // [n] x 16 B
+    unsigned* count = (unsigned*)((char*)d_work + np4 + (size_t)n * 32 + (((size_t)n * 16 + 255) & ~(size_t)255));
+    GRIDFF_CUDA(cudaMemsetAsync(count, 0, (size_t)n_bins * 4, st));
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    k_bin_count<<<blocks, 256, 0, st>>>(G, n, d_pos, nby, nbz, n_bins, count, rank);
+    GRIDFF_LAUNCH_CHECK("k_bin_count");
+    k_bin_scan<<<1, 1024, 0, st>>>(n_bins, count);
+    GRIDFF_LAUNCH_CHECK("k_bin_scan");
+    k_bin_scatter<<<blocks, 256, 0, st>>>(G, n, d_pos, (const float4*)d_coef, nby, nbz, n_bins, count, rank, rec);
+    GRIDFF_LAUNCH_CHECK("k_bin_scatter");
+    const long long per_block = kEvalWarps * 32;
+    cudaError_t e = launch_with_window(grid, k_eval_coop, dim3((unsigned)((n + per_block - 1) / per_block)), dim3(kEvalWarps * 32), 0, st, G, n, d_pos, (const float4*)d_coef,
+                                       d_E, d_F, (const unsigned*)nullptr, (const float4*)rec, out4);
+    count_launch();
+    if (e != cudaSuccess) return cuda_fail(e, "gridff_eval_binned launch");
+    k_bin_gather_out<<<blocks, 256, 0, st>>>(n, rank, out4, d_E, d_F);
+    GRIDFF_LAUNCH_CHECK("k_bin_gather_out");
+    return GRIDFF_OK;
 }
 
 size_t gridff_eval_work_bytes(long long n) {

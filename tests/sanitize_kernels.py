@@ -12,7 +12,7 @@ the 100-1000x slow-down of racecheck within minutes.  Modes reached (printed as 
   grid build        Morse per-node and tiled sampling (magnitude window on / off), Coulomb, prefilters, z-fastest and 4x4x4-brick stores,
                     gridff_grid_from_samples, export; derived stores: fp16, trilinear foil, micro-bricks x 1 / 2 / 8
   gridff_eval       variants 1 (thread per point), 2 (warp-cooperative LDG), 3 (3-D TMA box), the brick kernel, fp16, trilinear,
-                    micro-brick LDG gather and 5-D TMA box; the device-side kernel choice (classify + both kernels) on a store declared > L2
+                    micro-brick LDG gather and 5-D TMA box, gridff_eval_binned (count / scan / scatter / gather-back); the device-side kernel choice (classify + both kernels) on a store declared > L2
                     is reached through the same kernels; host-buffer pipeline
   k_replicas        <= 32 atoms on one warp: velocity Verlet variants 1, 2, 3, time-multiplexed VV and Langevin (state handed between
                     warps through global memory across __syncthreads), FIRE, FIRE + Philox restart + minima records, driven scan with a
@@ -86,6 +86,7 @@ def main():
             api.gridff_eval(g1, dp, dc, variant=v)
         api.gridff_eval(gb, dp, dc)
         api.gridff_eval(gs, dp, dc)
+        api.gridff_eval_binned(g1, dp, dc)
         for name, gd in derived.items():
             for v in ((0, 2, 3) if name == "bricks8" else (0, 2) if name.startswith("bricks") else (0,)):
                 api.gridff_eval(gd, dp, dc, variant=v)

@@ -62,6 +62,7 @@ def test_eval_kernels_under_schedule_stress(api, sapi):
         sp, sc = dp[order].contiguous(), dc[order].contiguous()
         for v in (1, 2, 3):
             out += list(A.gridff_eval(g, dp, dc, variant=v)) + list(A.gridff_eval(g, sp, sc, variant=v))
+        out += list(A.gridff_eval_binned(g, dp, dc))           # counting sort by atomics: the order inside a bin varies, the results must not
         for lay, variants in ((A.LAYOUT_HALF, (0,)), (A.LAYOUT_TRILINEAR, (0,)), (A.LAYOUT_MBRICK, (2,)), (A.LAYOUT_MBRICK2, (2,)), (A.LAYOUT_MBRICK8, (2, 3))):
             gd = A.gridff_grid_derive(g, lay)
             for v in variants:

@@ -143,6 +143,36 @@ def test_micro_brick_stores_match_zfast_and_oracle(api, orc, cfg1s, cfg3s, k):
         api.gridff_grid_export(stores[2][1])
 
 
+def test_eval_binned_matches_eval_bit_for_bit(api, cfg1s, cfg3s):
+    """gridff_eval_binned (counting sort of the points by blocks of 4 x 4 x 8 cells on the device, then the gather block by block, results written
+    to each point's own index; the path for scattered points on stores beyond the L2) returns gridff_eval's numbers bit for bit:
+    any point count (one point, less than a block, a ragged tail, many bins), wrapped coordinates, points below node 1 and above the domain (their
+    own bin), duplicates of one point (a bin far larger than a warp); twice in a row (the order inside a bin depends on the atomics, the results
+    do not)."""
+    for cfg in (cfg1s, cfg3s):
+        g = gpu_grid(api, cfg["sub"], cfg["desc"])
+        for n in (1, 33, 5000, 150011):
+            pos, coef = eval_points(cfg, n, 700 + n)
+            if n >= 5000:
+                pos[100:1100] = pos[100]                       # 1000 copies of one point
+                pos[2000:2100, 2] = 1e30                       # far above the domain
+            dp, dc = dev(pos), dev(coef)
+            E, F = api.gridff_eval(g, dp, dc, variant=2)
+            for _ in range(2):
+                Eb, Fb = api.gridff_eval_binned(g, dp, dc)
+                assert bool(torch.equal(E, Eb)) and bool(torch.equal(F, Fb)), n
+        need = api._lib.gridff_eval_binned_work_bytes(g.handle, n)
+        assert need >= 52 * n
+        with pytest.raises(api.GridffError) as e:
+            api.gridff_eval_binned(g, dp, dc, d_work=torch.empty(need - 1024, dtype=torch.uint8, device="cuda"))
+        assert e.value.code == api.ESIZE
+    gb = gpu_grid(api, cfg1s["sub"], cfg1s["desc"], layout=1)
+    with pytest.raises(api.GridffError):
+        api.gridff_eval_binned(gb, dp, dc)                     # brick layout: refused
+    E0, F0 = api.gridff_eval_binned(g, torch.zeros((0, 3), device="cuda"), torch.zeros((0, 4), device="cuda"))
+    assert E0.numel() == 0
+
+
 def test_derive_errors(api, cfg1s):
     g = gpu_grid(api, cfg1s["sub"], cfg1s["desc"])
     gb = gpu_grid(api, cfg1s["sub"], cfg1s["desc"], layout=1)
