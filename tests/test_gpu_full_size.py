@@ -108,6 +108,10 @@ def test_config4_full_size_sampled_points_and_order(api, orc):
     Eb, Fb = api.gridff_eval(gb, d_pos[perm].contiguous(), d_coef[perm].contiguous())
     assert bool(torch.equal(Eb, Es)) and bool(torch.equal(Fb, Fs))
     gb.free(); del gb, Eb, Fb
+    # gridff_eval_binned (device-side counting sort of the points by cell block) over the same 2^26 points: the same numbers
+    Eb, Fb = api.gridff_eval_binned(g, d_pos, d_coef)
+    assert bool(torch.equal(Eb, E)) and bool(torch.equal(Fb, F))
+    del Eb, Fb
     # the spatial sort did what it says: consecutive points share a cell far more often than in random order
     cell = lambda p: (torch.floor(p[:, 0] / d["Lx"] * 113) * 113 + torch.floor(p[:, 1] / d["Ly"] * 113)).long()
     c_s = cell(d_pos[perm][: 1 << 20]); c_r = cell(d_pos[: 1 << 20])

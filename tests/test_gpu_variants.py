@@ -151,7 +151,7 @@ def test_eval_binned_matches_eval_bit_for_bit(api, cfg1s, cfg3s):
     do not)."""
     for cfg in (cfg1s, cfg3s):
         g = gpu_grid(api, cfg["sub"], cfg["desc"])
-        for n in (1, 33, 5000, 150011):
+        for n in (1, 33, 5000, 150011, (1 << 20) + 77):
             pos, coef = eval_points(cfg, n, 700 + n)
             if n >= 5000:
                 pos[100:1100] = pos[100]                       # 1000 copies of one point
