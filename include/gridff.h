@@ -156,6 +156,21 @@ size_t gridff_eval_binned_work_bytes(const gridff_grid* grid, long long n);
 int gridff_eval_binned(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
                        float* d_E, float* d_F, void* d_work, size_t work_bytes, void* cuda_stream);
 
+/* gridff_eval_binned for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc): the
+ * same passes and the same numbers, bit for bit, with the work space in a device array built into the library — GRIDFF_NOALLOC_SCRATCH_BYTES
+ * (16 MiB) of every GPU that loads the library, held until the process exits.  The call allocates nothing: no cudaMalloc / cudaFree, no allocating
+ * library routine; d_pos, d_coef, d_E, d_F are the caller's as in gridff_eval.  Limits: n <= GRIDFF_NOALLOC_MAX_POINTS (262,144) and
+ * gridff_eval_binned_work_bytes(grid, n) <= gridff_eval_binned_noalloc_max_bytes() (52 bytes per point + 4 per block of 4 x 4 x 8 cells: at the full
+ * point count that leaves 3.1 MB for the counters: grids up to 7.8e5 blocks = 1e8 cells, e.g. 512 x 512 x 256; larger grids take fewer points per call);
+ * beyond either, GRIDFF_ESIZE with the numbers in gridff_last_error() and nothing launched.  ALL calls on one device share the one array, which keeps
+ * the previous call's contents: the bin counters are cleared on the stream at the start of every call, everything else is written before it is read;
+ * two calls that overlap on the GPU (different streams, no dependency between them) race on it — order them on one stream or with events. */
+#define GRIDFF_NOALLOC_SCRATCH_BYTES (16u << 20)
+#define GRIDFF_NOALLOC_MAX_POINTS (1 << 18)
+size_t gridff_eval_binned_noalloc_max_bytes(void);
+int gridff_eval_binned_noalloc(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef,
+                               float* d_E, float* d_F, void* cuda_stream);
+
 /* Same through HOST buffers: copies pos/coef to d_work, evaluates, copies E/F back, synchronises the stream.
  * d_work needs gridff_eval_work_bytes(n) bytes.  The work is pipelined in chunks of 2^22 points over two library-owned copy streams
  * and the caller's stream (upload of chunk c+1, kernel of chunk c and download of chunk c-1 overlap); the overlap needs pinned

@@ -84,6 +84,8 @@ _SIG = {
     "gridff_eval_variant": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _i, _vp]),
     "gridff_eval_binned_work_bytes": (_sz, [_vp, _ll]),
     "gridff_eval_binned": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
+    "gridff_eval_binned_noalloc_max_bytes": (_sz, []),
+    "gridff_eval_binned_noalloc": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp]),
     "gridff_eval_work_bytes": (_sz, [_ll]),
     "gridff_eval_host": (_i, [_vp, _ll, _vp, _vp, _vp, _vp, _vp, _sz, _vp]),
     "gridff_molecule_bytes": (_sz, [_P(Topology)]),
@@ -284,6 +286,18 @@ def gridff_eval_binned(grid, d_pos, d_coef, d_E=None, d_F=None, d_work=None, str
     if d_work is None:
         d_work = _alloc(int(_lib.gridff_eval_binned_work_bytes(grid.handle, n)))
     _check(_lib.gridff_eval_binned(grid.handle, n, _dptr(d_pos), _dptr(d_coef), _dptr(d_E), _dptr(d_F), _dptr(d_work), d_work.numel(), _stream(stream)))
+    return d_E, d_F
+
+
+def gridff_eval_binned_noalloc_max_bytes():
+    return int(_lib.gridff_eval_binned_noalloc_max_bytes())
+
+
+def gridff_eval_binned_noalloc(grid, d_pos, d_coef, d_E, d_F, stream=None):
+    """gridff_eval_binned with its work space in a device array built into the library (16 MiB; at most 2^18 points per call): the call
+    allocates nothing, so the outputs are the caller's too.  Calls that overlap on the GPU race on the shared array.  Returns (d_E, d_F)."""
+    n = d_pos.shape[0]
+    _check(_lib.gridff_eval_binned_noalloc(grid.handle, n, _dptr(d_pos), _dptr(d_coef), _dptr(d_E), _dptr(d_F), _stream(stream)))
     return d_E, d_F
 
 

@@ -363,6 +363,56 @@ int gridff_eval_binned(const gridff_grid* grid, long long n, const float* d_pos,
     return GRIDFF_OK;
 }
 
+}  // extern "C"
+
+// ---- gridff_eval_binned_noalloc: the same passes with their work space in a file-scope device array (callers that cannot allocate) ----
+// In host code `g_binned_scratch` is only a host-side stand-in for the symbol, never a device address: binned_scratch_ptr() asks the runtime for
+// the device address once per device (with that device current) and the entry point hands that pointer to the kernels.
+constexpr size_t kNoAllocScratchBytes = (size_t)GRIDFF_NOALLOC_SCRATCH_BYTES;
+static __device__ __align__(256) unsigned char g_binned_scratch[kNoAllocScratchBytes];
+constexpr int kNoAllocMaxDevices = 64;
+static std::atomic<void*> g_binned_scratch_ptr[kNoAllocMaxDevices];
+
+static int binned_scratch_ptr(void** out) {
+    int dev = -1;
+    GRIDFF_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) { set_error("device ordinal %d outside the %d the no-alloc path keeps addresses for", dev, kNoAllocMaxDevices); return GRIDFF_EUNSUPPORTED; }
+    void* p = g_binned_scratch_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        cudaError_t e = cudaGetSymbolAddress(&p, g_binned_scratch);      // the address on the CURRENT device; two racing threads store the same value
+        if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_binned_scratch)");
+        if (!p || ((uintptr_t)p & 255)) { set_error("the scratch symbol resolved to an unusable address"); return GRIDFF_ECUDA; }
+        g_binned_scratch_ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return GRIDFF_OK;
+}
+
+extern "C" {
+
+size_t gridff_eval_binned_noalloc_max_bytes(void) { return kNoAllocScratchBytes; }
+
+int gridff_eval_binned_noalloc(const gridff_grid* grid, long long n, const float* d_pos, const float* d_coef, float* d_E, float* d_F, void* cuda_stream) {
+    if (!grid) { set_error("grid is NULL"); return GRIDFF_EINVAL; }
+    if (n < 0) { set_error("n < 0"); return GRIDFF_EINVAL; }
+    if (n > (long long)GRIDFF_NOALLOC_MAX_POINTS) {
+        set_error("gridff_eval_binned_noalloc takes at most %lld points per call (got %lld): split the batch or use gridff_eval_binned with your own work space",
+                  (long long)GRIDFF_NOALLOC_MAX_POINTS, n);
+        return GRIDFF_ESIZE;
+    }
+    const size_t need = gridff_eval_binned_work_bytes(grid, n);
+    if (need > kNoAllocScratchBytes) {
+        set_error("gridff_eval_binned_noalloc: %lld points on this grid need %zu bytes of work space, the built-in scratch holds %zu (4 bytes per block of 4x4x8 cells + 52 per point)",
+                  n, need, kNoAllocScratchBytes);
+        return GRIDFF_ESIZE;
+    }
+    void* scratch = nullptr;
+    int rc = binned_scratch_ptr(&scratch);
+    if (rc) return rc;
+    // the same passes as gridff_eval_binned over the built-in scratch; its bin counters are cleared there (cudaMemsetAsync on the stream) on every call
+    return gridff_eval_binned(grid, n, d_pos, d_coef, d_E, d_F, scratch, kNoAllocScratchBytes, cuda_stream);
+}
+
 size_t gridff_eval_work_bytes(long long n) {
     if (n < 0) n = 0;
     return (size_t)n * (12 + 16 + 4 + 12) + 256;
