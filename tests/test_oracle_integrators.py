@@ -214,3 +214,51 @@ def test_fire_restart_records_minima(orc, small_grid):
             p0 = orc.restart_conformation(t, integ, g.Lx, g.Ly, r, k)
             solo = orc.run_replicas(g, t, orc.make_integrator("fire", 40000, 0.5, f_tol=1e-3), p0[None], np.zeros((1, 12, 3)))
             assert np.abs(solo["pos"][0] - m[4:].reshape(12, 3)).max() < 1e-12
+
+
+def test_fire_schedule_on_a_constant_force(orc):
+    """FIRE's time-step schedule pinned on the one case where it has a closed form: one atom on a potential that is linear in z (a
+    B-spline with node values -g z reproduces it exactly), started at rest.  The force is constant, so v stays parallel to F (the mixing
+    leaves it unchanged) and P = F.v > 0 from the second iteration on; the positions then depend on the schedule alone:
+        x_n - x_0 = c sum_{i<=n} dt_i sum_{j<=i} dt_j ,
+    with dt_i from the published rule (Bitzek et al. 2006, PAPER.md ref 72, as read in DESIGN.md R13): P <= 0 (the first iteration, v = 0)
+    halves dt and zeroes v; once "the number of steps since P was negative is LARGER than N_min" dt grows by f_inc per iteration up to
+    dt_max; the update of dt precedes the Euler step of the same iteration.  Ratios to the first displacement remove the unit constant c.
+    An off-by-one in the N_min test, a dt update after the step, or a missing reset at P = 0 each change these ratios by percents."""
+    nx = ny = 8; nz = 80; h = 0.1; z0 = 1.0; g = 0.05
+    z = z0 + h * np.arange(nz)
+    coef = np.broadcast_to((-g * z)[None, None, :, None], (nx, ny, nz, 1)).copy()
+    og = orc.OracleGrid(coef, nx * h, ny * h, z0, h)
+    topo = dict(n_atoms=1, mass=np.array([12.0]), q=np.zeros(1), lj_e=np.zeros(1), lj_R=np.ones(1),
+                bond=np.zeros((0, 2)), bond_k_r0=np.zeros((0, 2)), angle=np.zeros((0, 3)), angle_k_t0=np.zeros((0, 2)),
+                tors=np.zeros((0, 4)), tors_k_n_p0=np.zeros((0, 3)), excl=np.ones((1, 1), np.uint8))
+    t = orc.OracleTopology(topo, np.array([[1.0, 0.0, 0.0, 0.0]]))
+    x0 = np.array([[[0.33, 0.41, 2.0]]])
+    E, F = orc.forces(og, t, x0[0])[:2]
+    assert np.allclose(F, [[0.0, 0.0, g]], atol=1e-12)                      # the constant force
+    dt0, n_min, f_inc, f_dec, n = 0.5, 5, 1.1, 0.5, 40
+    dt_max = 3.0 * dt0                                                      # reached inside the run: the cap is exercised too
+    xs = []
+    for k in range(1, n + 1):
+        o = orc.run_replicas(og, t, orc.make_integrator("fire", k, dt0, f_tol=1e-9, dt_max=dt_max, n_min=n_min, f_inc=f_inc, f_dec=f_dec),
+                             x0, np.zeros_like(x0))
+        assert o["status"][0, 1] == 0 and o["status"][0, 0] == k
+        assert np.allclose(o["pos"][0, 0, :2], x0[0, 0, :2], atol=1e-15)
+        xs.append(o["pos"][0, 0, 2] - x0[0, 0, 2])
+    # the schedule written out from the rule
+    dts, dt, npos = [], dt0, 0
+    for i in range(1, n + 1):
+        if i == 1:                                    # v = 0: P = 0 is not > 0
+            dt *= f_dec; npos = 0
+        else:
+            npos += 1
+            if npos > n_min:
+                dt = min(dt * f_inc, dt_max)
+        dts.append(dt)
+    dts = np.array(dts)
+    assert dts[6] == dts[0] * f_inc and dts[5] == dts[0] and dts[-1] == dt_max
+    expect = np.cumsum(dts * np.cumsum(dts)) / dts[0] ** 2
+    got = np.array(xs) / xs[0]
+    assert np.allclose(got, expect, rtol=1e-10), np.abs(got / expect - 1).max()
+    # and the unit constant itself: x_1 - x_0 = dt_1^2 (g / m) * 9.648533e-3 Å/fs² per eV/(Å amu)  (CODATA: e / u * 1e-20... = 0.964853e-2)
+    assert abs(xs[0] / (dts[0] ** 2 * g / 12.0) - 9.64853e-3) < 1e-7
