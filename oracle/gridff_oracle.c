@@ -20,7 +20,7 @@
  *   force field      textbook 2/3/4-atom cases, FD, zero net force/torque     pinned
  *   velocity Verlet  harmonic-diatomic closed forms, reversibility            pinned
  *   FIRE             quadratic-bowl minimum, launch-split invariance;         pinned
- *                    time-step schedule: closed form on a constant force
+ *                    time-step schedule and mixing order: closed forms on a constant force
  *   Philox4x32-10    brute-force big-integer restatement in Python            pinned
  *   restart geometry bond lengths/angles invariant under torsion moves        pinned
  *   Langevin (BAOAB) gamma = 0 -> velocity Verlet, exact OU decay and equilibrium

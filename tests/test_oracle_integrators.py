@@ -262,3 +262,38 @@ def test_fire_schedule_on_a_constant_force(orc):
     assert np.allclose(got, expect, rtol=1e-10), np.abs(got / expect - 1).max()
     # and the unit constant itself: x_1 - x_0 = dt_1^2 (g / m) * 9.648533e-3 Å/fs² per eV/(Å amu)  (CODATA: e / u * 1e-20... = 0.964853e-2)
     assert abs(xs[0] / (dts[0] ** 2 * g / 12.0) - 9.64853e-3) < 1e-7
+
+
+def test_fire_mixing_order_on_a_constant_force(orc):
+    """The velocity mixing pinned the same way: constant force along z, initial velocity with a component ACROSS it.  The Euler step never
+    touches v_x and the mixing v <- (1 - a) v + a |v| F/|F| shrinks it by exactly (1 - a), so the lateral path depends only on the order
+    of the operations and on the schedules of a and dt (Bitzek et al. 2006, PAPER.md ref 72 / DESIGN.md R13: force, P = F.v, mixing with
+    the CURRENT a, then — after more than N_min steps with P > 0 — dt <- min(dt f_inc, dt_max) and a <- a f_a, then the step with the new
+    dt and the mixed velocity):      x_n - x_0 = v_x0 sum_{i<=n} dt_i prod_{j<=i} (1 - a_j).
+    Mixing after the step, mixing with the updated a, or stepping with the old dt each change the sum in its leading digits."""
+    nx = ny = 8; nz = 120; h = 0.1; z0 = 1.0; g = 0.05
+    z = z0 + h * np.arange(nz)
+    coef = np.broadcast_to((-g * z)[None, None, :, None], (nx, ny, nz, 1)).copy()
+    og = orc.OracleGrid(coef, nx * h, ny * h, z0, h)
+    topo = dict(n_atoms=1, mass=np.array([12.0]), q=np.zeros(1), lj_e=np.zeros(1), lj_R=np.ones(1),
+                bond=np.zeros((0, 2)), bond_k_r0=np.zeros((0, 2)), angle=np.zeros((0, 3)), angle_k_t0=np.zeros((0, 2)),
+                tors=np.zeros((0, 4)), tors_k_n_p0=np.zeros((0, 3)), excl=np.ones((1, 1), np.uint8))
+    t = orc.OracleTopology(topo, np.array([[1.0, 0.0, 0.0, 0.0]]))
+    x0 = np.array([[[0.33, 0.41, 2.0]]]); v0 = np.array([[[2.0e-3, 0.0, 1.0e-3]]])           # Å/fs; F.v > 0 from the first iteration
+    dt0, n_min, f_inc, a_start, f_a, n = 0.5, 5, 1.1, 0.1, 0.99, 30
+    dt_max = 2.0 * dt0
+    dt, a, npos, vx, x, expect = dt0, a_start, 0, v0[0, 0, 0], 0.0, []
+    for i in range(1, n + 1):
+        vx *= 1.0 - a                                  # mixing with the current a
+        npos += 1
+        if npos > n_min:
+            dt = min(dt * f_inc, dt_max); a *= f_a
+        x += dt * vx                                   # the step: new dt, mixed velocity
+        expect.append(x)
+    for k in (1, 2, 5, 6, 7, 12, n):
+        o = orc.run_replicas(og, t, orc.make_integrator("fire", k, dt0, f_tol=1e-9, dt_max=dt_max, n_min=n_min, f_inc=f_inc, a_start=a_start, f_a=f_a),
+                             x0, v0)
+        assert o["status"][0, 0] == k and o["status"][0, 1] == 0
+        got = o["pos"][0, 0, 0] - x0[0, 0, 0]
+        assert abs(got / expect[k - 1] - 1.0) < 1e-11, (k, got, expect[k - 1])
+        assert o["pos"][0, 0, 1] == x0[0, 0, 1]
