@@ -221,8 +221,8 @@ def test_defective_substrate_grid_and_eval(api, orc):
 
 
 def test_morse_window_is_exact(api, orc, cfg1s):
-    """The magnitude-window Morse sampling (terms more than e^-46 below a node's largest term skipped; used for large image blocks such
-    as config 3's) must give the same fp32 coefficients as the full sum, and the oracle's."""
+    """The tiled Morse sampling (per block of nodes: terms more than e^-34 below the block's largest term dropped, those more than e^-17 below it
+    summed in fp32; gridff_build.cu) must give the same fp32 coefficients as the full fp64 sum, and the oracle's."""
     og, _ = oracle_grid(orc, cfg1s["sub"], cfg1s["desc"])
     out = {}
     for flag, mw in (("0", 2), ("1", 1)):                    # gridff_grid_desc.morse_window: 2 = never, 1 = always
