@@ -233,3 +233,69 @@ def test_fire_restart_basins_config2(api, orc):
     # every recorded GPU minimum really is one (statement 3): stationary under the oracle's forces, the oracle's energy, stays put
     rec = np.array([kg[c] for c in sorted(kg)][:24])
     assert_true_minima(orc, og, ot, rec[:, 4:].reshape(len(rec), n, 3), rec[:, 3], 1e-3, "config 2 records")
+
+
+def test_fire_schedule_and_mixing_closed_forms_gpu(api):
+    """The CUDA path's FIRE against the closed forms the oracle is pinned to (tests/test_oracle_integrators.py), with no oracle in between: one
+    atom on a potential linear in z (imported samples V = -g z on a grid whose nodes and values are exact in fp32: the spline reproduces it, the
+    force is the constant g).  From rest: z_n - z_0 = c (g / m) sum_i dt_i sum_{j<=i} dt_j with dt_i from the published schedule (reset at
+    P = 0 in the first iteration, growth once more than N_min steps had P > 0, cap at dt_max).  With a velocity across the force:
+    x_n - x_0 = v_x0 sum_i dt_i prod_{j<=i} (1 - a_j).  fp32 state: 2e-6 Å + 1e-5 relative."""
+    h, nx, nz, z0, g, m = 0.125, 8, 64, 1.0, 2.0, 1.0
+    desc = api.make_desc(nx * h, nx * h, 0.0, z0, z0 + nz * h, h, 1.6, [api.CH_PAULI])
+    dims, _, _ = api.gridff_grid_dims(desc)
+    assert dims == (nx, nx, nz)
+    z = z0 + h * np.arange(nz)
+    samples = np.broadcast_to((-g * z)[None, None, :, None], (nx, nx, nz, 1)).astype(np.float32)
+    grid = api.gridff_grid_from_samples(desc, dev(samples))
+    topo = dict(n_atoms=1, mass=np.array([m]), q=np.zeros(1), lj_e=np.zeros(1), lj_R=np.ones(1),
+                bond=np.zeros((0, 2)), bond_k_r0=np.zeros((0, 2)), angle=np.zeros((0, 3)), angle_k_t0=np.zeros((0, 2)),
+                tors=np.zeros((0, 4)), tors_k_n_p0=np.zeros((0, 3)), excl=np.ones((1, 1), np.uint8))
+    mol = api.gridff_create_molecule(topo, np.array([[1.0, 0.0, 0.0, 0.0]], np.float32))
+    n_rep = 37
+    rng = np.random.default_rng(3)
+    x0 = np.zeros((n_rep, 1, 3), np.float32)
+    x0[:, 0, :2] = rng.uniform(0.0, nx * h, (n_rep, 2)); x0[:, 0, 2] = 2.0
+    c = 9.64853321e-3                                  # Å/fs² per eV/(Å amu): e / u (CODATA 2018) in these units
+    dt0, n_min, f_inc, f_dec, a_start, f_a, n = 0.25, 5, 1.3, 0.5, 0.1, 0.99, 20
+    dt_max = 2.0 * dt0
+    kw = dict(f_tol=1e-9, dt_max=dt_max, n_min=n_min, f_inc=f_inc, f_dec=f_dec, a_start=a_start, f_a=f_a)
+    # (1) from rest
+    dts, dt, npos = [], dt0, 0
+    for i in range(1, n + 1):
+        if i == 1:
+            dt *= f_dec; npos = 0                      # v = 0: P = 0 is not > 0
+        else:
+            npos += 1
+            if npos > n_min:
+                dt = min(dt * f_inc, dt_max)
+        dts.append(dt)
+    dts = np.array(dts)
+    assert dts[-1] == dt_max and dts[6] == dts[0] * f_inc
+    expect = c * g / m * np.cumsum(dts * np.cumsum(dts))
+    for k in (1, 2, 6, 7, 8, 12, n):
+        dp, dv = dev(x0), dev(np.zeros_like(x0))
+        out = api.gridff_run_replicas(grid, mol, api.make_integrator("fire", k, dt0, **kw), dp, dv)
+        torch.cuda.synchronize()
+        st = out["status"].cpu().numpy()
+        assert np.all(st[:, 0] == k) and np.all(st[:, 1] == 0)
+        p = dp.cpu().numpy().astype(np.float64)
+        assert np.abs(p[:, 0, :2] - x0[:, 0, :2]).max() <= 1e-6       # no lateral force beyond fp32 rounding of the weights' derivative sum
+        dz = p[:, 0, 2] - 2.0
+        assert np.abs(dz - expect[k - 1]).max() <= 2e-6 + 1e-5 * expect[k - 1], (k, dz[:3], expect[k - 1])
+    # (2) a velocity across the force
+    v0 = np.zeros_like(x0); v0[:, 0, 0] = 2.0e-3; v0[:, 0, 2] = 1.0e-3
+    dt, a, npos, vx, x, lateral = dt0, a_start, 0, 2.0e-3, 0.0, []
+    for i in range(1, n + 1):
+        vx *= 1.0 - a                                  # mixing with the current a
+        npos += 1
+        if npos > n_min:
+            dt = min(dt * f_inc, dt_max); a *= f_a
+        x += dt * vx                                   # the step: new dt, mixed velocity
+        lateral.append(x)
+    for k in (1, 5, 6, 7, n):
+        dp, dv = dev(x0), dev(v0)
+        api.gridff_run_replicas(grid, mol, api.make_integrator("fire", k, dt0, **kw), dp, dv)
+        torch.cuda.synchronize()
+        dx = dp.cpu().numpy().astype(np.float64)[:, 0, 0] - x0[:, 0, 0].astype(np.float64)
+        assert np.abs(dx - lateral[k - 1]).max() <= 1e-6 + 1e-5 * lateral[k - 1], (k, dx[:3], lateral[k - 1])
