@@ -233,11 +233,11 @@ int eval_tma(const gridff_grid* grid, long long n, const float* d_pos, const flo
     const size_t smem = kTmaWarps * ((kWarpSmem + 1023) & ~(size_t)1023) + 128;
     const bool bricks = grid->geom.n_copies == 8;
     auto kern = bricks ? k_eval_tma<true> : k_eval_tma<false>;
-    static bool attr_set[2] = {false, false};
-    if (!attr_set[bricks]) {
+    static bool attr_set[64][2] = {};                     // per device: function attributes belong to the device that is current when they are set
+    if (dev < 0 || dev >= 64 || !attr_set[dev][bricks]) {
         GRIDFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         GRIDFF_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
-        attr_set[bricks] = true;
+        if (dev >= 0 && dev < 64) attr_set[dev][bricks] = true;
     }
     int per_sm = 1;
     GRIDFF_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kTmaWarps * 32, smem));

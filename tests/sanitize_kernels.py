@@ -87,6 +87,7 @@ def main():
         api.gridff_eval(gb, dp, dc)
         api.gridff_eval(gs, dp, dc)
         api.gridff_eval_binned(g1, dp, dc)
+        api.gridff_eval_binned_noalloc(g1, dp, dc, torch.empty(n, device="cuda"), torch.empty((n, 3), device="cuda"))     # the same passes over the built-in scratch
         for name, gd in derived.items():
             for v in ((0, 2, 3) if name == "bricks8" else (0, 2) if name.startswith("bricks") else (0,)):
                 api.gridff_eval(gd, dp, dc, variant=v)
