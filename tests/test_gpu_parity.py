@@ -91,6 +91,27 @@ def test_grid_from_samples_reproduces_cubic(api):
     assert np.abs(Fn[:, 2] + dpoly).max() < 2e-3 and np.abs(Fn[:, :2]).max() < 2e-3
 
 
+@pytest.mark.parametrize("nx,ny,nz", [(5, 7, 8), (4, 4, 9), (9, 5, 31), (6, 11, 32), (7, 9, 33), (13, 4, 64), (5, 13, 65), (33, 31, 150)])
+def test_prefilter_edge_sizes_match_oracle(api, orc, nx, ny, nz):
+    """a3 on imported samples at sizes that straddle the prefilter kernels' blocking: line counts that are not a multiple of 32 (the z pass moves
+    32 lines per warp through a shared tile), z lengths of 8 (the smallest the tiled pass takes), one less / equal / one more than a 32-element
+    chunk, several chunks with a ragged tail; x and y lengths that are not a multiple of the cyclic pass's batches of 8.  Coefficients against the
+    oracle's dense solve of the same fp32 samples: half an fp32 ulp plus 1e-6 of the scale (random samples: the prefilter amplifies, no cancellation
+    is spared)."""
+    rng = np.random.default_rng(nx * 10000 + ny * 100 + nz)
+    samples = rng.normal(size=(nx, ny, nz, 2)).astype(np.float32)
+    h = 0.1
+    d = api.make_desc(nx * h, ny * h, 0.0, 1.5, 1.5 + nz * h, h, 1.6, [api.CH_PAULI, api.CH_LONDON])
+    dims, _, _ = api.gridff_grid_dims(d)
+    assert dims == (nx, ny, nz)
+    g = api.gridff_grid_from_samples(d, dev(samples))
+    coef = api.gridff_grid_export(g).cpu().numpy().astype(np.float64)
+    ref = orc.prefilter(samples.astype(np.float64), (1, 1, 0))
+    assert coef.shape == ref.shape
+    err = np.abs(coef - ref)
+    assert np.all(err <= 6.0e-8 * np.abs(ref) + 1e-9 * np.abs(ref).max()), (err.max(), np.abs(ref).max())
+
+
 # ------------------------------------------------------------------------------------------------ interpolation (a5)
 
 def eval_points(cfg, n, seed, rng_z=(1.55, 8.6)):
