@@ -284,3 +284,24 @@ def test_adatom_and_z_ref_rule_of_the_coulomb_channel(api, orc):
     # a Morse-only grid has no such rule
     g2 = gpu_grid(api, sub, inputs.grid_desc(Lx, Ly, 0.0, 1.5, 6.5, 0.2, 1.6, [inputs.PAULI, inputs.LONDON]))
     assert g2.info()["n_channels"] == 2
+
+
+def test_morse_grid_with_a_node_on_an_atom(api, orc):
+    """A Morse-only grid may reach into the substrate (no z_ref rule there): with z_lo = 0 the lowest node plane is the top atomic layer and the
+    node at a top-layer atom's x, y sits ON the atom — distance exactly 0.  The sampling's own square root (reciprocal-square-root seed) must
+    return 0 there, not NaN: coefficients finite and the oracle's, to the usual half fp32 ulp, over the whole grid."""
+    sub, Lx, Ly = inputs.rocksalt_slab(2, 3, 2.82, 0.0)
+    top = sub["pos"][np.isclose(sub["pos"][:, 2], sub["pos"][:, 2].max())]
+    desc = inputs.grid_desc(Lx, Ly, float(sub["pos"][:, 2].max()), 0.0, 1.2, 0.2, 1.6, [inputs.PAULI, inputs.LONDON])
+    nx, ny, nz = inputs.grid_dims(desc)
+    hx, hy = Lx / nx, Ly / ny
+    on_node = [(a[0] / hx, a[1] / hy) for a in top if abs(a[0] / hx - round(a[0] / hx)) < 1e-12 and abs(a[1] / hy - round(a[1] / hy)) < 1e-12]
+    assert len(on_node) >= 1, "the case needs a top-layer atom on a node of plane 0"
+    og, samples = oracle_grid(orc, sub, desc)
+    assert np.all(np.isfinite(samples))
+    g = gpu_grid(api, sub, desc)
+    coef = api.gridff_grid_export(g).cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(coef))
+    for ch in range(2):
+        ref = og.coef[..., ch]
+        assert np.all(np.abs(coef[..., ch] - ref) <= 6.0e-8 * np.abs(ref) + 1e-9 * np.abs(ref).max()), ch
