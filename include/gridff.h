@@ -74,7 +74,9 @@ typedef struct {
     int n_channels;       /* 1..4; every node is stored as 4 floats (16 B), missing channels are zero                    */
     int channel[4];       /* gridff_channel per stored component                                                        */
     int layout;           /* gridff_layout                                                                              */
-    int l2_persist;       /* 1: ask for an L2 access-policy window over the store on the streams that use the grid      */
+    int l2_persist;       /* 1: ask for an L2 access-policy window over the store on the streams that use the grid; honoured
+                             only when the store fits the device's largest persisting carve-out (a window that cannot hold the
+                             store costs the HBM-bound gathers 10-19 %: DESIGN.md §5) */
     int morse_window;     /* Morse sampling (a1): 0 = library's choice, 1 = always skip the terms below fp64 rounding of the node's
                              sum (the magnitude window), 2 = never (every image term is evaluated); same coefficients  */
 } gridff_grid_desc;
